@@ -1,0 +1,166 @@
+/* rte.h — C ABI of the B200-native pseudospectral P_N radiative-transport time stepper.
+ *
+ * The library advances the spherical-harmonic (3-D) / circular-harmonic (2-D) moment fields psi_c(r,t) of the
+ * radiative transport equation (eq.(1)) on a periodic Fourier-collocation grid:
+ *
+ *     psi_c^{n+1}(r) = psi_c^n(r) - c dt ( T_c(r) + sigma_l(r) psi_c^n(r) ) + c dt 1_Omega(r) q_c(r, t_n)
+ *
+ *     T      = sum_axis A_axis D_axis psi        streaming operator s.grad of eq.(6)/(10)
+ *     D_axis = IDFT_axis( i k_axis DFT_axis(.) ) spectral derivative, eq.(7)-(8)
+ *     sigma_l= mu_a + mu_s (1 - g^l)  in Omega   Henyey-Greenstein diagonal mu_t - mu_s g^l, eq.(5),(9)
+ *            = mu_b                   in the PML eq.(12); half-cosine profile of PAPER.md:165
+ *     step   = forward Euler                     eq.(11), PAPER.md:104 (signs per DESIGN.md reading R3)
+ *
+ * All of it runs in hand-written sm_100a kernels; there is no CPU fallback: every call that needs the device
+ * returns RTE_ECUDA when no CUDA device / wrong architecture is present.
+ *
+ * Conventions
+ *   units            mm, ps, mm^-1 (as the paper)
+ *   grid             nx*ny*nz cells, x fastest; cell i along an axis sits at (i - n/2) dx; nz = 1 when dim = 2.
+ *                    Every extent must be one of 16,32,48,64,96,128,192,256,384,512.
+ *   coefficients     3-D: C=(N+1)^2, c = l*l + l + m; m>=0 is the cos-type real harmonic a_l^m, m<0 the sin-type
+ *                    b_l^|m| (R6).  2-D: C=2N+1, c=0 -> a_0, c=2m-1 -> a_m, c=2m -> b_m (R8).
+ *                    Coefficient 0 is the fluence in both (R9).
+ *   field layout     external arrays are [c][z][y][x] fp32, contiguous (x fastest).
+ *   pointers         "_dev" arguments are CUDA device pointers (e.g. torch.Tensor.data_ptr()) valid on the context's
+ *                    device; "_host" arguments are host pointers (pinned memory makes the copies asynchronous).
+ *                    The library never frees caller memory.  It keeps the workspace and the stream until
+ *                    rte_destroy; every other array is consumed (stream-ordered) during the call.
+ *   stream           all work is enqueued on the cudaStream_t passed to rte_create (NULL = legacy default
+ *                    stream); calls return without synchronising unless stated.
+ *   errors           every function returns an rte status; nothing throws or aborts across the ABI.
+ *                    rte_last_error gives a text for the last failure on that context.
+ */
+#ifndef RTE_H_
+#define RTE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rte_ctx rte_ctx; /* opaque; owned by the library, freed by rte_destroy */
+
+enum { RTE_OK = 0, RTE_EINVAL = 1, RTE_ENOMEM = 2, RTE_ECUDA = 3, RTE_ESTATE = 4, RTE_EUNSUPPORTED = 5 };
+
+typedef struct {
+    int dim;        /* 2 or 3 */
+    int nx, ny, nz; /* nz = 1 when dim = 2 */
+} rte_grid;
+
+/* Perfectly matched layer, eq.(12) PAPER.md:113-119.  width = cells per side (0 = fully periodic, no layer).
+ * Depth of cell i along an axis: p = max(width - i, i - (n-1-width), 0); delta = max over axes of p / width;
+ * mu_b = mu_lo + (mu_hi - mu_lo) (1 - cos(pi delta))/2 for delta > 0 (half-cosine; R11).
+ * In the layer sigma_l = mu_b for every l, mu_s = 0 and q = 0.  Requires 2*width < every extent. */
+typedef struct {
+    int width;
+    float mu_lo, mu_hi; /* mm^-1 */
+} rte_pml;
+
+/* Optical properties of eq.(1)-(2).  Each pointer is a DEVICE pointer to either 1 value (is_map = 0) or
+ * nx*ny*nz values in [z][y][x] order (is_map = 1).  Values inside the PML are ignored. */
+typedef struct {
+    const float *mu_a, *mu_s, *g;
+    int mu_a_is_map, mu_s_is_map, g_is_map;
+} rte_media;
+
+/* ---- host-only helpers (no device needed) ------------------------------------------------------------------ */
+
+/* Number of real coefficient fields C: (N+1)^2 in 3-D, 2N+1 in 2-D (R8). <0 on bad input. */
+int rte_num_coeffs(int dim, int N);
+
+/* Real-basis streaming coupling of eq.(6)/(10) (R1, R7, R8):
+ * A_out[c*C + c'] (host, C*C doubles) with T_c = sum_c' A[c][c'] d psi_c' / d x_axis; axis 0=x, 1=y, 2=z. */
+int rte_coupling_table(int dim, int N, int axis, double* A_out_host);
+
+/* Bytes of device workspace rte_create needs for this grid and order (state, partial sums, coefficient maps). */
+int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out);
+
+/* ---- life cycle ---------------------------------------------------------------------------------------------- */
+
+/* Build a solver: validates, generates the coupling tables, wavenumbers (k at Nyquist = 0, R5), FFT
+ * twiddles and the per-cell sigma / PML maps on the device, zeroes the state, sets t = 0.
+ * workspace_dev: caller-owned device memory of at least rte_workspace_bytes, 256-byte aligned, alive until
+ * rte_destroy.  cuda_stream: a cudaStream_t (may be NULL).
+ * RTE_EINVAL: N<1, dx/dt/c <= 0, unsupported extent, dim/grid mismatch, PML too wide, workspace too small or
+ * misaligned.  RTE_ECUDA: no sm_100 device or a CUDA failure.  The time step is NOT checked for stability
+ * (the paper chooses dt "by inspection"). */
+int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx_mm, float dt_ps, float c_mm_per_ps,
+               const rte_media* media, const rte_pml* pml, void* workspace_dev, size_t workspace_bytes,
+               void* cuda_stream);
+void rte_destroy(rte_ctx* ctx);
+
+/* ---- state ----------------------------------------------------------------------------------------------------- */
+
+/* Set / read all moment fields, [C][nz][ny][nx] fp32.  An initial radiance distribution is how a delta(t) pulse
+ * enters.  rte_set_state does not reset the clock; rte_reset_time does. */
+int rte_set_state(rte_ctx* ctx, const float* psi_dev);
+int rte_get_state(rte_ctx* ctx, float* psi_dev);
+int rte_set_state_host(rte_ctx* ctx, const float* psi_host); /* host -> device inside the call, stream-ordered */
+int rte_get_state_host(rte_ctx* ctx, float* psi_host);       /* device -> host, synchronises the stream       */
+int rte_reset_time(rte_ctx* ctx);
+
+/* Source term q_c(r,t) = w[c] * S(r) * f(t) of eq.(1),(4), added as c dt q(t_n) each step
+ * (eq.(11); R3, R14) and only inside Omega (eq.(12)).
+ * w_host: C angular weights (host).  S: spatial footprint on the box [origin, origin+extent) in cells, laid out
+ * [bz][by][bx]; *_dev takes a device pointer, *_host a host pointer.  temporal_kind: 0 none (clears the source),
+ * 1 constant f = 1, 2 Gaussian f = exp(-(t-t0)^2 / (2 sigma_t^2)). */
+int rte_set_source(rte_ctx* ctx, const float* w_host, const float* S_dev, const int box_origin[3],
+                   const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps);
+int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, const int box_origin[3],
+                        const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps);
+
+/* ---- the hot path ---------------------------------------------------------------------------------------------- */
+
+/* Advance nsteps forward-Euler steps (eq.(11)); asynchronous on the stream.  One step = one pencil-FFT kernel per
+ * axis (DFT -> i k -> IDFT -> coupling), the last one fused with scattering, PML, source and the integrator. */
+int rte_step(rte_ctx* ctx, int nsteps);
+
+/* Same as rte_step, but brackets every per-axis kernel with CUDA events on the context's stream and returns the
+ * accumulated device time per axis in milliseconds (ms_axis_host[3], host; unused axes get 0) and the number of
+ * launches per axis actually timed (may be NULL).  Synchronises the stream before returning. */
+int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host);
+
+/* Fluence Phi(r) = coefficient 0 (eq.(3) normalisation; R9) over the whole grid, PML
+ * cells included, [nz][ny][nx] fp32. */
+int rte_fluence(rte_ctx* ctx, float* phi_dev);
+int rte_fluence_host(rte_ctx* ctx, float* phi_host); /* device -> host, synchronises the stream */
+
+/* Relative L2 change of the fluence over Omega since the previous call of this function (inf on the first call):
+ * the steady-state test of configs[3] (R17).  Synchronises the stream. */
+int rte_fluence_change(rte_ctx* ctx, double* rel_change_out);
+
+int rte_time_ps(const rte_ctx* ctx, double* t_out);  /* t = steps taken since the last reset * dt */
+int rte_sync(rte_ctx* ctx);                          /* stream synchronise; surfaces deferred CUDA errors */
+const char* rte_last_error(const rte_ctx* ctx);      /* ctx may be NULL: text of the last failed rte_create */
+
+/* Number of kernels the library has launched on this context so far (bench.py's gpu_launches claim). */
+int rte_launch_count(const rte_ctx* ctx, long long* count_out);
+
+/* ---- geometry / coefficient layer (device generators for heterogeneous media; north_star item (3)) ------------- */
+
+/* Fill mu_a/mu_s/g maps ([z][y][x], device) with a background and n_ell axis-aligned ellipsoids (disks in 2-D),
+ * later ones overwriting earlier ones.  ell_host: n_ell rows of 9 floats
+ * {cx, cy, cz, ax, ay, az, mu_a, mu_s, g}: centre and semi-axes in mm in the grid frame (cell i at (i-n/2) dx).
+ * A cell belongs to an ellipsoid when sum ((r-c)/a)^2 <= 1 (z term dropped in 2-D).  Any of the three output
+ * pointers may be NULL. */
+int rte_media_ellipsoids(const rte_grid* grid, float dx_mm, const float background[3], int n_ell,
+                         const float* ell_host, float* mu_a_dev, float* mu_s_dev, float* g_dev, void* cuda_stream);
+
+/* Smooth log-normal field: out = exp(ln(mean) - sigma_log^2/2 + sigma_log f), f = unit-variance periodic Gaussian
+ * random field with covariance exp(-r^2/(2 corr_len^2)): white noise (counter-based generator)
+ * circularly convolved with a separable Gaussian of std corr_len/sqrt2 per axis, renormalised to unit sample
+ * variance.  scratch_dev: nx*ny*nz floats of device scratch. */
+int rte_media_lognormal(const rte_grid* grid, float dx_mm, uint64_t seed, float mean, float sigma_log,
+                        float corr_len_mm, float* out_dev, float* scratch_dev, void* cuda_stream);
+
+/* The PML profile alone (mu_b per cell, 0 inside Omega) and the Omega mask (1 inside), device outputs. */
+int rte_pml_profile(const rte_grid* grid, const rte_pml* pml, float* mu_b_dev, unsigned char* inside_dev,
+                    void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RTE_H_ */

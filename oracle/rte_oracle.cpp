@@ -453,6 +453,56 @@ static void one_step(Oracle* o, int formulation) {
 // ------------------------------------------------------------------------------------------------------------
 // C interface for the ctypes wrapper (oracle/rte_oracle.py)
 // ------------------------------------------------------------------------------------------------------------
+// One cell of one step, computed on its own (see orc_step_cell below).
+template <typename Real>
+static void step_cell_impl(void* h, const Real* psi, int x, int y, int z, double* out /*[C]*/) {
+    Oracle* o = (Oracle*)h;
+    const int C = o->C; const long G = o->G;
+    const int n[3] = {o->nx, o->ny, o->nz};
+    const long st[3] = {1, o->nx, (long)o->nx * o->ny};
+    const int pos[3] = {x, y, z};
+    const long cell = ((long)z * o->ny + y) * o->nx + x;
+    std::vector<double> D((size_t)3 * C, 0.0);
+    for (int a = 0; a < o->dim; ++a) {
+        const int na = n[a];
+        std::vector<double> k(na), d(na, 0.0);
+        wavenumbers(na, o->dx, k.data());
+        for (int r = 0; r < na; ++r) {
+            double acc = 0;
+            for (int q = 0; q < na; ++q) acc += -k[q] * std::sin(2.0 * PI * (double)((long)q * r % na) / (double)na);
+            d[r] = acc / (double)na;
+        }
+        const long base = cell - pos[a] * st[a];
+        for (int cp = 0; cp < C; ++cp) {
+            double acc = 0;
+            for (int j = 0; j < na; ++j) acc += d[((pos[a] - j) % na + na) % na] * (double)psi[(size_t)cp * G + base + j * st[a]];
+            D[(size_t)a * C + cp] = acc;
+        }
+    }
+    const double cdt = o->c * o->dt;
+    const double ft = source_time(o, (double)o->step_count * o->dt);
+    for (int c = 0; c < C; ++c) {
+        double T = 0;
+        for (int a = 0; a < o->dim; ++a)
+            for (int cp = 0; cp < C; ++cp) T += o->A[a][(size_t)c * C + cp] * D[(size_t)a * C + cp];
+        double sigma;
+        if (o->inside[cell]) {
+            double gl = 1.0;
+            for (int j = 0; j < o->L[c]; ++j) gl *= o->g[cell];
+            sigma = o->mu_a[cell] + o->mu_s[cell] * (1.0 - gl);
+        } else sigma = o->mu_b[cell];
+        const double p = (double)psi[(size_t)c * G + cell];
+        double v = p - cdt * (T + sigma * p);
+        if (o->src_kind != 0 && o->inside[cell]) {
+            const int bx = x - o->src_org[0], by = y - o->src_org[1], bz = z - o->src_org[2];
+            if (bx >= 0 && by >= 0 && bz >= 0 && bx < o->src_ext[0] && by < o->src_ext[1] && bz < o->src_ext[2])
+                v += cdt * o->src_w[c] * o->src_S[((size_t)bz * o->src_ext[1] + by) * o->src_ext[0] + bx] * ft;
+        }
+        out[c] = v;
+    }
+}
+
+
 extern "C" {
 
 int orc_num_threads(void) {
@@ -595,51 +645,10 @@ void orc_streaming(void* h, int formulation, double* T_out) {
 // psi_new[c] (all C) at cell (x,y,z) from the state psi ([C][nz][ny][nx], fp64), using the direct O(n) circulant
 // sum of D_a along the three pencils through the cell:  (D_a f)[i] = sum_j d[(i-j) mod n] f[j],
 // d[r] = (1/n) sum_k i k_a[k] exp(2 pi i k r / n)  (real, antisymmetric).
-void orc_step_cell(void* h, const double* psi, int x, int y, int z, double* out /*[C]*/) {
-    Oracle* o = (Oracle*)h;
-    const int C = o->C; const long G = o->G;
-    const int n[3] = {o->nx, o->ny, o->nz};
-    const long st[3] = {1, o->nx, (long)o->nx * o->ny};
-    const int pos[3] = {x, y, z};
-    const long cell = ((long)z * o->ny + y) * o->nx + x;
-    std::vector<double> D((size_t)3 * C, 0.0);
-    for (int a = 0; a < o->dim; ++a) {
-        const int na = n[a];
-        std::vector<double> k(na), d(na, 0.0);
-        wavenumbers(na, o->dx, k.data());
-        for (int r = 0; r < na; ++r) {
-            double acc = 0;
-            for (int q = 0; q < na; ++q) acc += -k[q] * std::sin(2.0 * PI * (double)((long)q * r % na) / (double)na);
-            d[r] = acc / (double)na;
-        }
-        const long base = cell - pos[a] * st[a];
-        for (int cp = 0; cp < C; ++cp) {
-            double acc = 0;
-            for (int j = 0; j < na; ++j) acc += d[((pos[a] - j) % na + na) % na] * psi[(size_t)cp * G + base + j * st[a]];
-            D[(size_t)a * C + cp] = acc;
-        }
-    }
-    const double cdt = o->c * o->dt;
-    const double ft = source_time(o, (double)o->step_count * o->dt);
-    for (int c = 0; c < C; ++c) {
-        double T = 0;
-        for (int a = 0; a < o->dim; ++a)
-            for (int cp = 0; cp < C; ++cp) T += o->A[a][(size_t)c * C + cp] * D[(size_t)a * C + cp];
-        double sigma;
-        if (o->inside[cell]) {
-            double gl = 1.0;
-            for (int j = 0; j < o->L[c]; ++j) gl *= o->g[cell];
-            sigma = o->mu_a[cell] + o->mu_s[cell] * (1.0 - gl);
-        } else sigma = o->mu_b[cell];
-        const double p = psi[(size_t)c * G + cell];
-        double v = p - cdt * (T + sigma * p);
-        if (o->src_kind != 0 && o->inside[cell]) {
-            const int bx = x - o->src_org[0], by = y - o->src_org[1], bz = z - o->src_org[2];
-            if (bx >= 0 && by >= 0 && bz >= 0 && bx < o->src_ext[0] && by < o->src_ext[1] && bz < o->src_ext[2])
-                v += cdt * o->src_w[c] * o->src_S[((size_t)bz * o->src_ext[1] + by) * o->src_ext[0] + bx] * ft;
-        }
-        out[c] = v;
-    }
-}
+// One cell of one step, computed on its own (for sampled parity at sizes where a whole oracle step is too slow):
+// psi_new[c] (all C) at cell (x,y,z) from the state psi ([C][nz][ny][nx]), using the direct O(n) circulant sum of D_a
+// along the three pencils through the cell.  The _f32 variant reads an fp32 state (values promoted to fp64).
+void orc_step_cell(void* h, const double* psi, int x, int y, int z, double* out) { step_cell_impl<double>(h, psi, x, y, z, out); }
+void orc_step_cell_f32(void* h, const float* psi, int x, int y, int z, double* out) { step_cell_impl<float>(h, psi, x, y, z, out); }
 
 }  // extern "C"

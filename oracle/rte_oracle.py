@@ -48,6 +48,7 @@ def lib():
         L.orc_time_ps.argtypes = [C.c_void_p]
         L.orc_streaming.argtypes = [C.c_void_p, C.c_int, dp]
         L.orc_step_cell.argtypes = [C.c_void_p, dp, C.c_int, C.c_int, C.c_int, dp]
+        L.orc_step_cell_f32.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int, C.c_int, C.c_int, dp]
         _lib = L
     return _lib
 
@@ -203,7 +204,10 @@ class Oracle:
 
     def step_cell(self, psi, x, y, z):
         """psi_new[:, z, y, x] after one step from state `psi` (fp64 [C,nz,ny,nx]), computed for that cell alone."""
-        psi = _f64(psi)
         out = np.zeros(self.C)
-        lib().orc_step_cell(self.h, _dp(psi), int(x), int(y), int(z), _dp(out))
+        if psi.dtype == np.float32 and psi.flags["C_CONTIGUOUS"]:
+            lib().orc_step_cell_f32(self.h, psi.ctypes.data_as(C.POINTER(C.c_float)), int(x), int(y), int(z), _dp(out))
+        else:
+            psi = _f64(psi)
+            lib().orc_step_cell(self.h, _dp(psi), int(x), int(y), int(z), _dp(out))
         return out

@@ -1,0 +1,185 @@
+// rte_fft.cuh — register-resident complex DFTs of small fixed size for the pencil-FFT kernels (sm_100a).
+//
+// The spectral derivative of PAPER.md eq.(7)-(8),(10) needs DFT_n / IDFT_n along a pencil with
+// n = N1*N2.  Each thread computes whole N1- or N2-point transforms in registers; everything here is fully
+// unrolled at compile time, twiddle factors are compile-time immediates (FFMA/FMUL immediate forms), and the
+// "natural order in, natural order out" contract makes the index bookkeeping of the callers trivial (the output
+// permutation of the Cooley-Tukey split is a register renaming, i.e. free).
+//
+// Forward sign: X[k] = sum_j x[j] exp(-2 pi i j k / R)   (eq.(8): exp(-i k.r)).
+// Inverse (unnormalised) = swap(re,im) o forward o swap(re,im), also free of instructions.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+#ifndef RTE_HD
+#define RTE_HD __host__ __device__ __forceinline__
+#endif
+
+namespace rtefft {
+
+// ---- compile-time cos/sin of 2 pi num/den (double precision Taylor series after octant reduction) ---------------
+constexpr double kTwoPi = 6.283185307179586476925286766559005768;
+
+__host__ __device__ constexpr double taylor_sin(double x) {  // |x| <= pi/4
+    double x2 = x * x, term = x, sum = x;
+    for (int i = 1; i < 14; ++i) { term *= -x2 / (double)((2 * i) * (2 * i + 1)); sum += term; }
+    return sum;
+}
+__host__ __device__ constexpr double taylor_cos(double x) {  // |x| <= pi/4
+    double x2 = x * x, term = 1.0, sum = 1.0;
+    for (int i = 1; i < 14; ++i) { term *= -x2 / (double)((2 * i - 1) * (2 * i)); sum += term; }
+    return sum;
+}
+// cos(2 pi f) for f in [0,1)
+__host__ __device__ constexpr double cos_turn(double f) {
+    if (f > 0.5) f = 1.0 - f;                   // cos symmetric about half a turn
+    if (f > 0.25) return -cos_turn(0.5 - f);    // second quadrant
+    if (f <= 0.125) return taylor_cos(kTwoPi * f);
+    return taylor_sin(kTwoPi * (0.25 - f));
+}
+__host__ __device__ constexpr double cos2pi(int num, int den) {
+    int r = ((num % den) + den) % den;
+    return cos_turn((double)r / (double)den);
+}
+__host__ __device__ constexpr double sin2pi(int num, int den) {    // sin(2 pi x) = cos(2 pi (x - 1/4))
+    return cos2pi(4 * num - den, 4 * den);
+}
+
+RTE_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+RTE_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+RTE_HD float2 cmul(float2 a, float2 w) {   // a * w
+    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.y, w.x, a.x * w.y));
+}
+RTE_HD float2 cmulc(float2 a, float2 w) {  // a * conj(w)
+    return make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(-a.x, w.y, a.y * w.x));
+}
+
+// a * exp(-2 pi i NUM/DEN) with the multiples of an eighth turn special-cased
+template <int NUM, int DEN>
+RTE_HD float2 mulw(float2 a) {
+    constexpr int r = ((NUM % DEN) + DEN) % DEN;
+    constexpr float h = 0.70710678118654752440f;
+    if constexpr (r == 0) return a;
+    else if constexpr (4 * r == DEN) return make_float2(a.y, -a.x);                       // * -i
+    else if constexpr (2 * r == DEN) return make_float2(-a.x, -a.y);                      // * -1
+    else if constexpr (4 * r == 3 * DEN) return make_float2(-a.y, a.x);                   // * +i
+    else if constexpr (8 * r == DEN) return make_float2((a.x + a.y) * h, (a.y - a.x) * h);        // (1-i)/sqrt2
+    else if constexpr (8 * r == 3 * DEN) return make_float2((a.y - a.x) * h, -(a.x + a.y) * h);   // (-1-i)/sqrt2
+    else if constexpr (8 * r == 5 * DEN) return make_float2(-(a.x + a.y) * h, (a.x - a.y) * h);   // (-1+i)/sqrt2
+    else if constexpr (8 * r == 7 * DEN) return make_float2((a.x - a.y) * h, (a.x + a.y) * h);    // (1+i)/sqrt2
+    else {
+        constexpr float c = (float)cos2pi(r, DEN);
+        constexpr float s = (float)sin2pi(r, DEN);   // w = c - i s
+        return make_float2(fmaf(a.y, s, a.x * c), fmaf(-a.x, s, a.y * c));
+    }
+}
+
+// ---- DFT of R points held at v[0], v[S], v[2S], ...; natural order in and out --------------------------------------
+template <int R, int S>
+struct Dft;
+
+template <int S>
+struct Dft<1, S> {
+    static RTE_HD void run(float2*) {}
+};
+
+template <int S>
+struct Dft<2, S> {
+    static RTE_HD void run(float2* v) {
+        const float2 a = v[0], b = v[S];
+        v[0] = cadd(a, b);
+        v[S] = csub(a, b);
+    }
+};
+
+template <int S>
+struct Dft<3, S> {
+    static RTE_HD void run(float2* v) {
+        constexpr float hs3 = 0.86602540378443864676f;   // sqrt(3)/2
+        const float2 a = v[0], b = v[S], c = v[2 * S];
+        const float2 s = cadd(b, c), d = csub(b, c);
+        const float2 m = make_float2(fmaf(-0.5f, s.x, a.x), fmaf(-0.5f, s.y, a.y));
+        // X1 = m - i hs3 d ; X2 = m + i hs3 d
+        v[0] = cadd(a, s);
+        v[S] = make_float2(fmaf(hs3, d.y, m.x), fmaf(-hs3, d.x, m.y));
+        v[2 * S] = make_float2(fmaf(-hs3, d.y, m.x), fmaf(hs3, d.x, m.y));
+    }
+};
+
+template <int S>
+struct Dft<4, S> {
+    static RTE_HD void run(float2* v) {
+        const float2 a = v[0], b = v[S], c = v[2 * S], d = v[3 * S];
+        const float2 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = csub(b, d);
+        v[0] = cadd(t0, t2);
+        v[2 * S] = csub(t0, t2);
+        v[S] = make_float2(t1.x + t3.y, t1.y - t3.x);       // t1 - i t3
+        v[3 * S] = make_float2(t1.x - t3.y, t1.y + t3.x);   // t1 + i t3
+    }
+};
+
+// first factor of the Cooley-Tukey split R = RA * RB
+template <int R>
+struct Split {
+    static constexpr int RA = (R % 3 == 0) ? 3 : ((R == 8) ? 2 : ((R % 4 == 0) ? 4 : 2));
+    static constexpr int RB = R / RA;
+};
+
+template <int RA, int RB, int S, int KA, int B>
+struct TwiddleRow {   // v[(RB*KA + b)*S] *= W_R^{b*KA} for b = B..RB-1
+    static RTE_HD void run(float2* v) {
+        if constexpr (B < RB) {
+            v[(RB * KA + B) * S] = mulw<B * KA, RA * RB>(v[(RB * KA + B) * S]);
+            TwiddleRow<RA, RB, S, KA, B + 1>::run(v);
+        }
+    }
+};
+template <int RA, int RB, int S, int KA>
+struct TwiddleAll {
+    static RTE_HD void run(float2* v) {
+        if constexpr (KA < RA) {
+            TwiddleRow<RA, RB, S, KA, 1>::run(v);
+            TwiddleAll<RA, RB, S, KA + 1>::run(v);
+        }
+    }
+};
+
+// generic: x[j], j = RB*a + b ; X[ka + RA*kb]
+//   step 1: for each b, DFT_RA over a (stride RB*S)          -> slot (RB*ka + b) holds Y[ka][b]
+//   step 2: slot (RB*ka + b) *= W_R^{b ka}
+//   step 3: for each ka, DFT_RB over b (stride S)             -> slot (RB*ka + kb) holds X[ka + RA*kb]
+//   step 4: un-permute (register renaming)
+template <int R, int S>
+struct Dft {
+    static constexpr int RA = Split<R>::RA, RB = Split<R>::RB;
+    static RTE_HD void run(float2* v) {
+#pragma unroll
+        for (int b = 0; b < RB; ++b) Dft<RA, RB * S>::run(v + b * S);
+        TwiddleAll<RA, RB, S, 1>::run(v);
+#pragma unroll
+        for (int ka = 0; ka < RA; ++ka) Dft<RB, S>::run(v + ka * RB * S);
+        float2 t[R];
+#pragma unroll
+        for (int ka = 0; ka < RA; ++ka)
+#pragma unroll
+            for (int kb = 0; kb < RB; ++kb) t[ka + RA * kb] = v[(RB * ka + kb) * S];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k * S] = t[k];
+    }
+};
+
+template <int R>
+RTE_HD void dft_fwd(float2 (&v)[R]) {
+    Dft<R, 1>::run(v);
+}
+template <int R>
+RTE_HD void dft_inv(float2 (&v)[R]) {   // unnormalised inverse
+#pragma unroll
+    for (int i = 0; i < R; ++i) { const float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
+    Dft<R, 1>::run(v);
+#pragma unroll
+    for (int i = 0; i < R; ++i) { const float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
+}
+
+}  // namespace rtefft

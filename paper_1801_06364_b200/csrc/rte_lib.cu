@@ -1,0 +1,868 @@
+// rte_lib.cu — C-ABI implementation (include/rte.h) of the B200-native P_N pseudospectral RTE stepper.
+// Host logic + the non-hot kernels (layout transposes, coefficient maps, geometry generators, reductions);
+// the hot per-axis pencil kernel lives in rte_pass.cuh, the register FFTs in rte_fft.cuh, the tables in rte_tables.h.
+// No CPU fallback anywhere: every entry point that computes does so in a CUDA kernel or fails with RTE_ECUDA.
+#include "../../include/rte.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "rte_pass.cuh"
+#include "rte_tables.h"
+
+using rtepass::CplEntry;
+using rtepass::PassArgs;
+
+namespace {
+
+thread_local char g_create_error[256] = "";
+
+struct AxisTables {
+    float2* tw = nullptr;
+    float* kap = nullptr;
+    CplEntry* cpl = nullptr;
+    int* cpl_cnt = nullptr;
+    int n = 0, N1 = 0, N2 = 0;
+};
+
+}  // namespace
+
+struct rte_ctx {
+    rte_grid grid{};
+    rte_pml pml{};
+    int N = 0, C = 0, Cp = 0, P = 0;
+    long long G = 0;
+    float dx = 0, dt = 0, c = 0;
+    cudaStream_t stream = nullptr;
+    // views into the caller's workspace
+    float2* psi = nullptr;
+    float2* part = nullptr;
+    float *sa = nullptr, *ss = nullptr, *gm = nullptr;
+    // small library-owned device arrays
+    AxisTables ax[3];
+    int* deg = nullptr;
+    int* ext_of_slot = nullptr;
+    float* srcw = nullptr;
+    float* srcS = nullptr;
+    size_t srcS_cap = 0;
+    float* phi_prev = nullptr;
+    double* red = nullptr;         // 2 doubles for reductions
+    bool have_prev = false;
+    // source
+    int src_kind = 0;
+    int src_org[3] = {0, 0, 0}, src_ext[3] = {0, 0, 0};
+    double src_t0 = 0, src_sig = 1;
+    long long steps = 0;
+    long long launches = 0;
+    char err[256] = "";
+};
+
+namespace {
+
+int fail(rte_ctx* ctx, int code, const char* fmt, const char* detail = "") {
+    char* dst = ctx ? ctx->err : g_create_error;
+    snprintf(dst, 256, fmt, detail);
+    return code;
+}
+
+#define CUDA_TRY(ctx, expr)                                                              \
+    do {                                                                                 \
+        cudaError_t e__ = (expr);                                                        \
+        if (e__ != cudaSuccess) return fail(ctx, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e__)); \
+    } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool extent_ok(int n) { int a, b; return rtetab::split_of(n, a, b); }
+
+int padded_coeffs(int dim, int N) {
+    std::vector<int> e, d;
+    rtetab::slot_order(dim, N, e, d);
+    return (int)e.size();
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// non-hot kernels
+// ---------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int pml_depth(int i, int n, int W) {
+    int p = W - i;
+    const int q = i - (n - 1 - W);
+    if (q > p) p = q;
+    return p > 0 ? p : 0;
+}
+
+// sigma maps: sa = mu_a (Omega) | mu_b (PML); ss = mu_s (Omega) | 0 (PML); gm = g.  eq.(12).
+__global__ void k_build_maps(float* __restrict__ sa, float* __restrict__ ss, float* __restrict__ gm,
+                             const float* __restrict__ mu_a, const float* __restrict__ mu_s,
+                             const float* __restrict__ g, int a_map, int s_map, int g_map, int dim, int nx, int ny,
+                             int nz, int W, float mu_lo, float mu_hi) {
+    const long long G = (long long)nx * ny * nz;
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        int p = 0;
+        if (W > 0) {
+            p = max(pml_depth(x, nx, W), pml_depth(y, ny, W));
+            if (dim == 3) p = max(p, pml_depth(z, nz, W));
+        }
+        if (p == 0) {
+            sa[cell] = a_map ? mu_a[cell] : mu_a[0];
+            ss[cell] = s_map ? mu_s[cell] : mu_s[0];
+        } else {
+            const float delta = (float)p / (float)W;
+            sa[cell] = mu_lo + (mu_hi - mu_lo) * 0.5f * (1.0f - cospif(delta));
+            ss[cell] = 0.f;
+        }
+        gm[cell] = g_map ? g[cell] : g[0];
+    }
+}
+
+__global__ void k_pml_profile(float* __restrict__ mu_b, unsigned char* __restrict__ inside, int dim, int nx, int ny,
+                              int nz, int W, float mu_lo, float mu_hi) {
+    const long long G = (long long)nx * ny * nz;
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        int p = 0;
+        if (W > 0) {
+            p = max(pml_depth(x, nx, W), pml_depth(y, ny, W));
+            if (dim == 3) p = max(p, pml_depth(z, nz, W));
+        }
+        float v = 0.f;
+        if (p > 0) v = mu_lo + (mu_hi - mu_lo) * 0.5f * (1.0f - cospif((float)p / (float)W));
+        if (mu_b) mu_b[cell] = v;
+        if (inside) inside[cell] = p == 0 ? 1 : 0;
+    }
+}
+
+// external [C][G] -> internal [G][Cp].  One 32x32 tile of (cell, slot) per block through shared memory so both sides
+// are coalesced.
+__global__ void k_import(float* __restrict__ dst, const float* __restrict__ src, const int* __restrict__ ext_of_slot,
+                         long long G, int Cp) {
+    __shared__ float tile[32][33];
+    const long long cell0 = (long long)blockIdx.x * 32;
+    const int s0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {     // j: slot within tile, threadIdx.x: cell
+        const int s = s0 + j;
+        const long long cell = cell0 + threadIdx.x;
+        float v = 0.f;
+        if (s < Cp && cell < G) {
+            const int e = ext_of_slot[s];
+            if (e >= 0) v = src[(size_t)e * G + cell];
+        }
+        tile[j][threadIdx.x] = v;
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {     // j: cell within tile, threadIdx.x: slot
+        const int s = s0 + threadIdx.x;
+        const long long cell = cell0 + j;
+        if (s < Cp && cell < G) dst[(size_t)cell * Cp + s] = tile[threadIdx.x][j];
+    }
+}
+
+__global__ void k_export(float* __restrict__ dst, const float* __restrict__ src, const int* __restrict__ ext_of_slot,
+                         long long G, int Cp) {
+    __shared__ float tile[32][33];
+    const long long cell0 = (long long)blockIdx.x * 32;
+    const int s0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {     // j: cell, threadIdx.x: slot
+        const int s = s0 + threadIdx.x;
+        const long long cell = cell0 + j;
+        tile[j][threadIdx.x] = (s < Cp && cell < G) ? src[(size_t)cell * Cp + s] : 0.f;
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {     // j: slot, threadIdx.x: cell
+        const int s = s0 + j;
+        const long long cell = cell0 + threadIdx.x;
+        if (s < Cp && cell < G) {
+            const int e = ext_of_slot[s];
+            if (e >= 0) dst[(size_t)e * G + cell] = tile[threadIdx.x][j];
+        }
+    }
+}
+
+__global__ void k_fluence(float* __restrict__ phi, const float* __restrict__ psi, long long G, int Cp) {
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x)
+        phi[cell] = psi[(size_t)cell * Cp];
+}
+
+// source footprint copy with q = 0 outside Omega (eq.(12))
+__global__ void k_source_copy(float* __restrict__ dst, const float* __restrict__ src, int ox, int oy, int oz, int ex,
+                              int ey, int ez, int dim, int nx, int ny, int nz, int W) {
+    const int total = ex * ey * ez;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+        const int bx = i % ex, by = (i / ex) % ey, bz = i / (ex * ey);
+        int p = 0;
+        if (W > 0) {
+            p = max(pml_depth(ox + bx, nx, W), pml_depth(oy + by, ny, W));
+            if (dim == 3) p = max(p, pml_depth(oz + bz, nz, W));
+        }
+        dst[i] = p == 0 ? src[i] : 0.f;
+    }
+}
+
+// sum over Omega of (phi - prev)^2 and phi^2 ; then prev <- phi
+__global__ void k_fluence_change(const float* __restrict__ psi, float* __restrict__ prev, double* __restrict__ red,
+                                 const float* __restrict__ ss_unused, int dim, int nx, int ny, int nz, int W, int Cp) {
+    const long long G = (long long)nx * ny * nz;
+    double d2 = 0, n2 = 0;
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        int p = 0;
+        if (W > 0) {
+            p = max(pml_depth(x, nx, W), pml_depth(y, ny, W));
+            if (dim == 3) p = max(p, pml_depth(z, nz, W));
+        }
+        const float v = psi[(size_t)cell * Cp];
+        if (p == 0) {
+            const double d = (double)v - (double)prev[cell];
+            d2 += d * d;
+            n2 += (double)v * (double)v;
+        }
+        prev[cell] = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        d2 += __shfl_down_sync(0xffffffffu, d2, o);
+        n2 += __shfl_down_sync(0xffffffffu, n2, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&red[0], d2); atomicAdd(&red[1], n2); }
+}
+
+// ---- geometry generators -------------------------------------------------------------------------------------------
+__global__ void k_ellipsoids(float* __restrict__ mu_a, float* __restrict__ mu_s, float* __restrict__ g,
+                             const float* __restrict__ ell, int n_ell, float bg_a, float bg_s, float bg_g, int dim,
+                             int nx, int ny, int nz, float dx) {
+    const long long G = (long long)nx * ny * nz;
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        const float px = (float)(x - nx / 2) * dx, py = (float)(y - ny / 2) * dx, pz = (float)(z - nz / 2) * dx;
+        float va = bg_a, vs = bg_s, vg = bg_g;
+        for (int e = 0; e < n_ell; ++e) {
+            const float* E = ell + 9 * e;
+            const float ux = (px - E[0]) / E[3], uy = (py - E[1]) / E[4];
+            float d = ux * ux + uy * uy;
+            if (dim == 3) { const float uz = (pz - E[2]) / E[5]; d += uz * uz; }
+            if (d <= 1.0f) { va = E[6]; vs = E[7]; vg = E[8]; }
+        }
+        if (mu_a) mu_a[cell] = va;
+        if (mu_s) mu_s[cell] = vs;
+        if (g) g[cell] = vg;
+    }
+}
+
+// counter-based generator: splitmix64 finaliser of (seed, index); two 24-bit uniforms -> Box-Muller normal
+__device__ __forceinline__ unsigned long long splitmix64(unsigned long long x) {
+    x += 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    return x ^ (x >> 31);
+}
+__global__ void k_white_noise(float* __restrict__ out, long long G, unsigned long long seed) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < G; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long h = splitmix64(seed * 0x100000001B3ull + (unsigned long long)i);
+        const unsigned int a = (unsigned int)(h >> 40), b = (unsigned int)((h >> 16) & 0xFFFFFFu);
+        const float u1 = ((float)a + 1.0f) * (1.0f / 16777216.0f);      // (0,1]
+        const float u2 = (float)b * (1.0f / 16777216.0f);               // [0,1)
+        out[i] = sqrtf(-2.0f * logf(u1)) * cospif(2.0f * u2);
+    }
+}
+// circular 1-D convolution along one axis with a truncated Gaussian (weights normalised to sum 1)
+__global__ void k_blur_axis(float* __restrict__ dst, const float* __restrict__ src, int nx, int ny, int nz, int axis,
+                            int R, float inv2s2 /* 1/(2 s^2) in cells^-2 */) {
+    const long long G = (long long)nx * ny * nz;
+    const int n[3] = {nx, ny, nz};
+    const long long st[3] = {1, nx, (long long)nx * ny};
+    float wsum = 0.f;
+    for (int j = -R; j <= R; ++j) wsum += expf(-(float)(j * j) * inv2s2);
+    for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
+         cell += (long long)gridDim.x * blockDim.x) {
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int pos[3] = {x, (int)(r % ny), (int)(r / ny)};
+        const long long base = cell - pos[axis] * st[axis];
+        const int na = n[axis];
+        float acc = 0.f;
+        for (int j = -R; j <= R; ++j) {
+            int i = (pos[axis] + j) % na;
+            if (i < 0) i += na;
+            acc = fmaf(expf(-(float)(j * j) * inv2s2), src[base + i * st[axis]], acc);
+        }
+        dst[cell] = acc / wsum;
+    }
+}
+__global__ void k_moments(const float* __restrict__ f, long long G, double* __restrict__ red) {
+    double s = 0, s2 = 0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < G; i += (long long)gridDim.x * blockDim.x) {
+        const double v = f[i];
+        s += v; s2 += v * v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        s += __shfl_down_sync(0xffffffffu, s, o);
+        s2 += __shfl_down_sync(0xffffffffu, s2, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&red[0], s); atomicAdd(&red[1], s2); }
+}
+__global__ void k_lognormal_finish(float* __restrict__ f, long long G, const double* __restrict__ red, float mean,
+                                   float sigma_log) {
+    const double m = red[0] / (double)G;
+    const double var = red[1] / (double)G - m * m;
+    const float fm = (float)m, inv_sd = (float)(1.0 / sqrt(var));
+    const float mu = logf(mean) - 0.5f * sigma_log * sigma_log;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < G; i += (long long)gridDim.x * blockDim.x)
+        f[i] = expf(fmaf(sigma_log, (f[i] - fm) * inv_sd, mu));
+}
+
+int grid_for(long long n, int block) {
+    long long b = (n + block - 1) / block;
+    if (b > 148 * 16) b = 148 * 16;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+int check_grid(const rte_grid* g) {
+    if (!g) return RTE_EINVAL;
+    if (g->dim != 2 && g->dim != 3) return RTE_EINVAL;
+    if (g->dim == 2 && g->nz != 1) return RTE_EINVAL;
+    if (!extent_ok(g->nx) || !extent_ok(g->ny)) return RTE_EINVAL;
+    if (g->dim == 3 && !extent_ok(g->nz)) return RTE_EINVAL;
+    return RTE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// pass dispatch
+// ---------------------------------------------------------------------------------------------------------------------
+struct LaunchPlan { int TP, nt, blocks; size_t smem; };
+
+LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
+    const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz;
+    int groups = 1;
+    if (axis == 0) { A.stride_i = 1; A.stride_t = nx; A.group_stride = 0; A.pencils_per_group = ny * nz; }
+    else if (axis == 1) {
+        A.stride_i = nx; A.stride_t = 1; A.group_stride = nx * ny; A.pencils_per_group = nx; groups = nz;
+    } else { A.stride_i = nx * ny; A.stride_t = 1; A.group_stride = 0; A.pencils_per_group = nx * ny; }
+    const AxisTables& T = c->ax[axis];
+    const int P = c->P, n = T.n;
+    int tp = 1;
+    while (tp * P < 32 && tp < 8) tp *= 2;
+    while (tp > 1 && (size_t)n * tp * P * 8 > 96 * 1024) tp /= 2;
+    while (tp > 1 && tp > A.pencils_per_group) tp /= 2;
+    A.TP = tp; A.P = P;
+    A.tiles_per_group = (A.pencils_per_group + tp - 1) / tp;
+    const int Q = tp * P;
+    const int T1 = Q * T.N2, T2 = Q * T.N1;
+    int best = 128; double best_cost = 1e30;
+    for (int nt = 64; nt <= 320; nt += 32) {
+        if (nt > T1 && nt > T2 && nt > 64) break;
+        const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;
+        const double cost = w1 + w2;
+        if (cost <= best_cost + 1e-12) { best_cost = cost; best = nt; }
+    }
+    LaunchPlan L;
+    L.TP = tp; L.nt = best; L.blocks = groups * A.tiles_per_group;
+    L.smem = (size_t)n * Q * sizeof(float2) + (size_t)n * sizeof(float2) + (size_t)n * sizeof(float);
+    return L;
+}
+
+template <int N1, int N2, int MODE>
+cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
+    auto kern = rtepass::pass_kernel<N1, N2, MODE>;
+    static size_t configured = 0;
+    if (L.smem > 48 * 1024 && L.smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200 * 1024));
+        if (e != cudaSuccess) return e;
+        configured = 200 * 1024;
+    }
+    kern<<<L.blocks, L.nt, L.smem, s>>>(A);
+    return cudaGetLastError();
+}
+
+template <int MODE>
+cudaError_t launch_mode(int n, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
+    switch (n) {
+        case 16: return launch_one<4, 4, MODE>(A, L, s);
+        case 32: return launch_one<4, 8, MODE>(A, L, s);
+        case 48: return launch_one<4, 12, MODE>(A, L, s);
+        case 64: return launch_one<8, 8, MODE>(A, L, s);
+        case 96: return launch_one<8, 12, MODE>(A, L, s);
+        case 128: return launch_one<8, 16, MODE>(A, L, s);
+        case 192: return launch_one<12, 16, MODE>(A, L, s);
+        case 256: return launch_one<16, 16, MODE>(A, L, s);
+        case 384: return launch_one<24, 16, MODE>(A, L, s);
+        case 512: return launch_one<32, 16, MODE>(A, L, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+double source_time_factor(const rte_ctx* c, double t) {
+    if (c->src_kind == 1) return 1.0;
+    if (c->src_kind == 2) { const double u = (t - c->src_t0) / c->src_sig; return std::exp(-0.5 * u * u); }
+    return 0.0;
+}
+
+int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
+    const int naxes = c->grid.dim;
+    for (int axis = 0; axis < naxes; ++axis) {
+        PassArgs A{};
+        A.psi = c->psi; A.part = c->part; A.out = c->psi;
+        A.tw = c->ax[axis].tw; A.kap = c->ax[axis].kap; A.cpl = c->ax[axis].cpl; A.cpl_cnt = c->ax[axis].cpl_cnt;
+        A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
+        A.cdt = c->c * c->dt;
+        A.srcS = c->srcS; A.srcw = c->srcw;
+        for (int k = 0; k < 3; ++k) { A.src_org[k] = c->src_org[k]; A.src_ext[k] = c->src_ext[k]; }
+        A.src_amp = 0.f;
+        A.nx = c->grid.nx; A.ny = c->grid.ny;
+        const LaunchPlan L = plan_pass(c, axis, A);
+        const int mode = axis == 0 ? rtepass::MODE_FIRST : (axis == naxes - 1 ? rtepass::MODE_LAST : rtepass::MODE_MIDDLE);
+        cudaError_t e;
+        if (mode == rtepass::MODE_LAST) {
+            if (c->src_kind != 0)
+                A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, (double)c->steps * (double)c->dt));
+            e = launch_mode<rtepass::MODE_LAST>(c->ax[axis].n, A, L, c->stream);
+        } else if (mode == rtepass::MODE_FIRST) e = launch_mode<rtepass::MODE_FIRST>(c->ax[axis].n, A, L, c->stream);
+        else e = launch_mode<rtepass::MODE_MIDDLE>(c->ax[axis].n, A, L, c->stream);
+        if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
+        c->launches += 1;
+        if (ev) cudaEventRecord(ev[axis], c->stream);
+    }
+    c->steps += 1;
+    return RTE_OK;
+}
+
+template <typename T>
+cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t s) {
+    cudaError_t e = cudaMalloc((void**)dst, v.size() * sizeof(T) + 16);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return e;
+    return cudaStreamSynchronize(s);   // v is pageable and about to go out of scope
+}
+
+void free_ctx(rte_ctx* c) {
+    if (!c) return;
+    for (int a = 0; a < 3; ++a) {
+        cudaFree(c->ax[a].tw); cudaFree(c->ax[a].kap); cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_cnt);
+    }
+    cudaFree(c->deg); cudaFree(c->ext_of_slot); cudaFree(c->srcw); cudaFree(c->srcS); cudaFree(c->phi_prev);
+    cudaFree(c->red);
+    delete c;
+}
+
+int set_source_common(rte_ctx* ctx, const float* w_host, const float* S, bool S_on_host, const int org[3],
+                      const int ext[3], int kind, float t0, float sig) {
+    if (!ctx) return RTE_ESTATE;
+    if (kind < 0 || kind > 2) return fail(ctx, RTE_EINVAL, "temporal_kind must be 0, 1 or 2");
+    if (kind == 0) { ctx->src_kind = 0; return RTE_OK; }
+    if (!w_host || !S || !org || !ext) return fail(ctx, RTE_EINVAL, "null source argument");
+    if (kind == 2 && !(sig > 0)) return fail(ctx, RTE_EINVAL, "sigma_t must be positive");
+    const int n[3] = {ctx->grid.nx, ctx->grid.ny, ctx->grid.nz};
+    for (int a = 0; a < 3; ++a)
+        if (org[a] < 0 || ext[a] < 1 || org[a] + ext[a] > n[a]) return fail(ctx, RTE_EINVAL, "source box outside the grid");
+    const size_t cells = (size_t)ext[0] * ext[1] * ext[2];
+    if (cells > ctx->srcS_cap) {
+        cudaFree(ctx->srcS); ctx->srcS = nullptr; ctx->srcS_cap = 0;
+        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->srcS, cells * sizeof(float)));
+        ctx->srcS_cap = cells;
+    }
+    // angular weights in slot order
+    std::vector<int> eos, deg;
+    rtetab::slot_order(ctx->grid.dim, ctx->N, eos, deg);
+    std::vector<float> w(ctx->Cp, 0.f);
+    for (int s = 0; s < ctx->Cp; ++s) if (eos[s] >= 0) w[s] = w_host[eos[s]];
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->srcw, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    const float* S_dev = S;
+    float* tmp = nullptr;
+    if (S_on_host) {
+        CUDA_TRY(ctx, cudaMalloc((void**)&tmp, cells * sizeof(float)));
+        cudaError_t e = cudaMemcpyAsync(tmp, S, cells * sizeof(float), cudaMemcpyHostToDevice, ctx->stream);
+        if (e != cudaSuccess) { cudaFree(tmp); return fail(ctx, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e)); }
+        S_dev = tmp;
+    }
+    k_source_copy<<<grid_for((long long)cells, 256), 256, 0, ctx->stream>>>(
+        ctx->srcS, S_dev, org[0], org[1], org[2], ext[0], ext[1], ext[2], ctx->grid.dim, n[0], n[1], n[2],
+        ctx->pml.width);
+    ctx->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (tmp) { cudaStreamSynchronize(ctx->stream); cudaFree(tmp); }
+    if (e != cudaSuccess) return fail(ctx, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e));
+    for (int a = 0; a < 3; ++a) { ctx->src_org[a] = org[a]; ctx->src_ext[a] = ext[a]; }
+    ctx->src_kind = kind; ctx->src_t0 = t0; ctx->src_sig = sig;
+    return RTE_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================================
+// C ABI
+// =====================================================================================================================
+extern "C" {
+
+int rte_num_coeffs(int dim, int N) { return rtetab::num_coeffs(dim, N); }
+
+int rte_coupling_table(int dim, int N, int axis, double* A_out_host) {
+    const int C = rtetab::num_coeffs(dim, N);
+    if (C < 0 || axis < 0 || axis > 2 || !A_out_host) return RTE_EINVAL;
+    std::vector<double> A[3];
+    rtetab::coupling_real(dim, N, A);
+    std::memcpy(A_out_host, A[axis].data(), (size_t)C * C * sizeof(double));
+    return RTE_OK;
+}
+
+int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out) {
+    if (!bytes_out || check_grid(grid) != RTE_OK || N < 1) return RTE_EINVAL;
+    const size_t G = (size_t)grid->nx * grid->ny * grid->nz;
+    const size_t Cp = (size_t)padded_coeffs(grid->dim, N);
+    const size_t field = align_up(G * Cp * sizeof(float), 256), map = align_up(G * sizeof(float), 256);
+    *bytes_out = 2 * field + 3 * map;
+    return RTE_OK;
+}
+
+int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, float c, const rte_media* media,
+               const rte_pml* pml, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return fail(nullptr, RTE_EINVAL, "out is null");
+    *out = nullptr;
+    if (check_grid(grid) != RTE_OK) return fail(nullptr, RTE_EINVAL, "unsupported grid (dim 2|3; extents in {16,32,48,64,96,128,192,256,384,512}; nz=1 in 2-D)");
+    if (N < 1 || N > 31) return fail(nullptr, RTE_EINVAL, "N must be in 1..31");
+    if (!(dx > 0) || !(dt > 0) || !(c > 0)) return fail(nullptr, RTE_EINVAL, "dx, dt, c must be positive");
+    if (!media || !media->mu_a || !media->mu_s || !media->g) return fail(nullptr, RTE_EINVAL, "media pointers are null");
+    rte_pml pm{0, 0.f, 0.f};
+    if (pml) pm = *pml;
+    if (pm.width < 0) return fail(nullptr, RTE_EINVAL, "negative PML width");
+    {
+        int nmin = grid->nx < grid->ny ? grid->nx : grid->ny;
+        if (grid->dim == 3 && grid->nz < nmin) nmin = grid->nz;
+        if (2 * pm.width >= nmin) return fail(nullptr, RTE_EINVAL, "PML wider than half the grid");
+    }
+    size_t need = 0;
+    rte_workspace_bytes(grid, N, &need);
+    if (!workspace_dev || workspace_bytes < need) return fail(nullptr, RTE_EINVAL, "workspace too small");
+    if (((uintptr_t)workspace_dev & 255u) != 0) return fail(nullptr, RTE_EINVAL, "workspace must be 256-byte aligned");
+
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
+        return fail(nullptr, RTE_ECUDA, "no CUDA device (this library has no CPU fallback)");
+    if (major != 10) return fail(nullptr, RTE_ECUDA, "kernels are built for sm_100a only");
+
+    rte_ctx* ctx = new (std::nothrow) rte_ctx();
+    if (!ctx) return fail(nullptr, RTE_ENOMEM, "out of host memory");
+    ctx->grid = *grid; ctx->pml = pm; ctx->N = N;
+    ctx->C = rtetab::num_coeffs(grid->dim, N);
+    ctx->Cp = padded_coeffs(grid->dim, N);
+    ctx->P = ctx->Cp / 2;
+    ctx->G = (long long)grid->nx * grid->ny * grid->nz;
+    ctx->dx = dx; ctx->dt = dt; ctx->c = c;
+    ctx->stream = (cudaStream_t)cuda_stream;
+
+    const size_t field = align_up((size_t)ctx->G * ctx->Cp * sizeof(float), 256), map = align_up((size_t)ctx->G * sizeof(float), 256);
+    char* w = (char*)workspace_dev;
+    ctx->psi = (float2*)w; w += field;
+    ctx->part = (float2*)w; w += field;
+    ctx->sa = (float*)w; w += map;
+    ctx->ss = (float*)w; w += map;
+    ctx->gm = (float*)w;
+
+#define CREATE_TRY(expr)                                                                         \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess) {                                                                \
+            fail(nullptr, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e__));                       \
+            free_ctx(ctx);                                                                       \
+            return RTE_ECUDA;                                                                    \
+        }                                                                                        \
+    } while (0)
+
+    // tables
+    const int ext_n[3] = {grid->nx, grid->ny, grid->nz};
+    for (int a = 0; a < grid->dim; ++a) {
+        AxisTables& T = ctx->ax[a];
+        T.n = ext_n[a];
+        rtetab::split_of(T.n, T.N1, T.N2);
+        std::vector<float> tw, kap;
+        rtetab::twiddles(T.n, tw);
+        rtetab::kappa_over_n(T.n, dx, kap);
+        std::vector<float2> tw2(T.n);
+        for (int j = 0; j < T.n; ++j) tw2[j] = make_float2(tw[2 * j], tw[2 * j + 1]);
+        CREATE_TRY(upload(&T.tw, tw2, ctx->stream));
+        CREATE_TRY(upload(&T.kap, kap, ctx->stream));
+        std::vector<std::vector<rtetab::PairEntry>> pe;
+        rtetab::pair_coupling(grid->dim, N, a, pe);
+        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE, CplEntry{0, 0.f, 0.f, 0.f, 0.f});
+        std::vector<int> cnt(ctx->P, 0);
+        for (int p = 0; p < ctx->P; ++p) {
+            if ((int)pe[p].size() > rtepass::kMaxE) {
+                free_ctx(ctx);
+                return fail(nullptr, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
+            }
+            cnt[p] = (int)pe[p].size();
+            for (int e = 0; e < cnt[p]; ++e)
+                flat[(size_t)p * rtepass::kMaxE + e] = CplEntry{pe[p][e].src, pe[p][e].w00, pe[p][e].w01, pe[p][e].w10, pe[p][e].w11};
+        }
+        CREATE_TRY(upload(&T.cpl, flat, ctx->stream));
+        CREATE_TRY(upload(&T.cpl_cnt, cnt, ctx->stream));
+    }
+    {
+        std::vector<int> eos, deg;
+        rtetab::slot_order(grid->dim, N, eos, deg);
+        CREATE_TRY(upload(&ctx->ext_of_slot, eos, ctx->stream));
+        CREATE_TRY(upload(&ctx->deg, deg, ctx->stream));
+        std::vector<float> zw(ctx->Cp, 0.f);
+        CREATE_TRY(upload(&ctx->srcw, zw, ctx->stream));
+        CREATE_TRY(cudaMalloc((void**)&ctx->red, 2 * sizeof(double)));
+    }
+    // coefficient maps and zero state
+    k_build_maps<<<grid_for(ctx->G, 256), 256, 0, ctx->stream>>>(ctx->sa, ctx->ss, ctx->gm, media->mu_a, media->mu_s,
+                                                                media->g, media->mu_a_is_map, media->mu_s_is_map,
+                                                                media->g_is_map, grid->dim, grid->nx, grid->ny, grid->nz,
+                                                                pm.width, pm.mu_lo, pm.mu_hi);
+    ctx->launches += 1;
+    CREATE_TRY(cudaGetLastError());
+    CREATE_TRY(cudaMemsetAsync(ctx->psi, 0, field, ctx->stream));
+    CREATE_TRY(cudaMemsetAsync(ctx->part, 0, field, ctx->stream));
+#undef CREATE_TRY
+    *out = ctx;
+    return RTE_OK;
+}
+
+void rte_destroy(rte_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    free_ctx(ctx);
+}
+
+int rte_set_state(rte_ctx* ctx, const float* psi_dev) {
+    if (!ctx) return RTE_ESTATE;
+    if (!psi_dev) return fail(ctx, RTE_EINVAL, "null state pointer");
+    dim3 grid((unsigned)((ctx->G + 31) / 32), (unsigned)((ctx->Cp + 31) / 32)), block(32, 8);
+    k_import<<<grid, block, 0, ctx->stream>>>((float*)ctx->psi, psi_dev, ctx->ext_of_slot, ctx->G, ctx->Cp);
+    ctx->launches += 1;
+    CUDA_TRY(ctx, cudaGetLastError());
+    ctx->have_prev = false;
+    return RTE_OK;
+}
+
+int rte_get_state(rte_ctx* ctx, float* psi_dev) {
+    if (!ctx) return RTE_ESTATE;
+    if (!psi_dev) return fail(ctx, RTE_EINVAL, "null state pointer");
+    dim3 grid((unsigned)((ctx->G + 31) / 32), (unsigned)((ctx->Cp + 31) / 32)), block(32, 8);
+    k_export<<<grid, block, 0, ctx->stream>>>(psi_dev, (const float*)ctx->psi, ctx->ext_of_slot, ctx->G, ctx->Cp);
+    ctx->launches += 1;
+    CUDA_TRY(ctx, cudaGetLastError());
+    return RTE_OK;
+}
+
+// Host variants stage through the partial-sum buffer (free between steps), so no extra device memory is needed.
+int rte_set_state_host(rte_ctx* ctx, const float* psi_host) {
+    if (!ctx) return RTE_ESTATE;
+    if (!psi_host) return fail(ctx, RTE_EINVAL, "null state pointer");
+    const size_t bytes = (size_t)ctx->C * ctx->G * sizeof(float);
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->part, psi_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    return rte_set_state(ctx, (const float*)ctx->part);
+}
+
+int rte_get_state_host(rte_ctx* ctx, float* psi_host) {
+    if (!ctx) return RTE_ESTATE;
+    if (!psi_host) return fail(ctx, RTE_EINVAL, "null state pointer");
+    int rc = rte_get_state(ctx, (float*)ctx->part);
+    if (rc != RTE_OK) return rc;
+    const size_t bytes = (size_t)ctx->C * ctx->G * sizeof(float);
+    CUDA_TRY(ctx, cudaMemcpyAsync(psi_host, ctx->part, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    return RTE_OK;
+}
+
+int rte_reset_time(rte_ctx* ctx) {
+    if (!ctx) return RTE_ESTATE;
+    ctx->steps = 0;
+    return RTE_OK;
+}
+
+int rte_set_source(rte_ctx* ctx, const float* w_host, const float* S_dev, const int box_origin[3],
+                   const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps) {
+    return set_source_common(ctx, w_host, S_dev, false, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+}
+int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, const int box_origin[3],
+                        const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps) {
+    return set_source_common(ctx, w_host, S_host, true, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+}
+
+int rte_step(rte_ctx* ctx, int nsteps) {
+    if (!ctx) return RTE_ESTATE;
+    if (nsteps < 0) return fail(ctx, RTE_EINVAL, "negative step count");
+    for (int s = 0; s < nsteps; ++s) {
+        const int rc = one_step(ctx);
+        if (rc != RTE_OK) return rc;
+    }
+    return RTE_OK;
+}
+
+int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host) {
+    if (!ctx) return RTE_ESTATE;
+    if (nsteps < 0 || !ms_axis_host) return fail(ctx, RTE_EINVAL, "bad rte_step_profile argument");
+    const int naxes = ctx->grid.dim;
+    std::vector<cudaEvent_t> ev((size_t)nsteps * naxes + 1);
+    for (auto& e : ev) CUDA_TRY(ctx, cudaEventCreate(&e));
+    int rc = RTE_OK;
+    cudaEventRecord(ev[0], ctx->stream);
+    for (int s = 0; s < nsteps && rc == RTE_OK; ++s) rc = one_step(ctx, &ev[(size_t)s * naxes + 1]);
+    if (rc == RTE_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = fail(ctx, RTE_ECUDA, "CUDA: %s", "stream synchronise failed");
+    for (int a = 0; a < 3; ++a) { ms_axis_host[a] = 0.0; if (launches_axis_host) launches_axis_host[a] = 0; }
+    if (rc == RTE_OK)
+        for (int s = 0; s < nsteps; ++s)
+            for (int a = 0; a < naxes; ++a) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ev[(size_t)s * naxes + a], ev[(size_t)s * naxes + a + 1]);
+                ms_axis_host[a] += ms;
+                if (launches_axis_host) launches_axis_host[a] += 1;
+            }
+    for (auto& e : ev) cudaEventDestroy(e);
+    return rc;
+}
+
+int rte_fluence(rte_ctx* ctx, float* phi_dev) {
+    if (!ctx) return RTE_ESTATE;
+    if (!phi_dev) return fail(ctx, RTE_EINVAL, "null fluence pointer");
+    k_fluence<<<grid_for(ctx->G, 256), 256, 0, ctx->stream>>>(phi_dev, (const float*)ctx->psi, ctx->G, ctx->Cp);
+    ctx->launches += 1;
+    CUDA_TRY(ctx, cudaGetLastError());
+    return RTE_OK;
+}
+
+int rte_fluence_host(rte_ctx* ctx, float* phi_host) {
+    if (!ctx) return RTE_ESTATE;
+    if (!phi_host) return fail(ctx, RTE_EINVAL, "null fluence pointer");
+    int rc = rte_fluence(ctx, (float*)ctx->part);
+    if (rc != RTE_OK) return rc;
+    CUDA_TRY(ctx, cudaMemcpyAsync(phi_host, ctx->part, (size_t)ctx->G * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    return RTE_OK;
+}
+
+int rte_fluence_change(rte_ctx* ctx, double* rel_change_out) {
+    if (!ctx) return RTE_ESTATE;
+    if (!rel_change_out) return fail(ctx, RTE_EINVAL, "null output pointer");
+    if (!ctx->phi_prev) {
+        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->phi_prev, (size_t)ctx->G * sizeof(float)));
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->phi_prev, 0, (size_t)ctx->G * sizeof(float), ctx->stream));
+        ctx->have_prev = false;
+    }
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->red, 0, 2 * sizeof(double), ctx->stream));
+    k_fluence_change<<<grid_for(ctx->G, 256), 256, 0, ctx->stream>>>((const float*)ctx->psi, ctx->phi_prev, ctx->red,
+                                                                    nullptr, ctx->grid.dim, ctx->grid.nx, ctx->grid.ny,
+                                                                    ctx->grid.nz, ctx->pml.width, ctx->Cp);
+    ctx->launches += 1;
+    CUDA_TRY(ctx, cudaGetLastError());
+    double h[2] = {0, 0};
+    CUDA_TRY(ctx, cudaMemcpyAsync(h, ctx->red, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (!ctx->have_prev || !(h[1] > 0)) *rel_change_out = std::numeric_limits<double>::infinity();
+    else *rel_change_out = std::sqrt(h[0] / h[1]);
+    ctx->have_prev = true;
+    return RTE_OK;
+}
+
+int rte_time_ps(const rte_ctx* ctx, double* t_out) {
+    if (!ctx) return RTE_ESTATE;
+    if (!t_out) return RTE_EINVAL;
+    *t_out = (double)ctx->steps * (double)ctx->dt;
+    return RTE_OK;
+}
+
+int rte_sync(rte_ctx* ctx) {
+    if (!ctx) return RTE_ESTATE;
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    CUDA_TRY(ctx, cudaGetLastError());
+    return RTE_OK;
+}
+
+const char* rte_last_error(const rte_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+int rte_launch_count(const rte_ctx* ctx, long long* count_out) {
+    if (!ctx) return RTE_ESTATE;
+    if (!count_out) return RTE_EINVAL;
+    *count_out = ctx->launches;
+    return RTE_OK;
+}
+
+int rte_media_ellipsoids(const rte_grid* grid, float dx, const float background[3], int n_ell, const float* ell_host,
+                         float* mu_a_dev, float* mu_s_dev, float* g_dev, void* cuda_stream) {
+    if (!grid || (grid->dim != 2 && grid->dim != 3) || grid->nx < 1 || grid->ny < 1 || grid->nz < 1) return RTE_EINVAL;
+    if (!(dx > 0) || !background || n_ell < 0 || (n_ell > 0 && !ell_host)) return RTE_EINVAL;
+    for (int e = 0; e < n_ell; ++e)
+        for (int k = 3; k < 6; ++k)
+            if (!(ell_host[9 * e + k] > 0) && !(grid->dim == 2 && k == 5)) return RTE_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    float* ell_dev = nullptr;
+    if (cudaMalloc((void**)&ell_dev, (size_t)(n_ell > 0 ? n_ell : 1) * 9 * sizeof(float)) != cudaSuccess) return RTE_ECUDA;
+    if (n_ell > 0 && cudaMemcpyAsync(ell_dev, ell_host, (size_t)n_ell * 9 * sizeof(float), cudaMemcpyHostToDevice, s) != cudaSuccess) {
+        cudaFree(ell_dev);
+        return RTE_ECUDA;
+    }
+    const long long G = (long long)grid->nx * grid->ny * grid->nz;
+    k_ellipsoids<<<grid_for(G, 256), 256, 0, s>>>(mu_a_dev, mu_s_dev, g_dev, ell_dev, n_ell, background[0], background[1],
+                                                 background[2], grid->dim, grid->nx, grid->ny, grid->nz, dx);
+    cudaError_t e = cudaGetLastError();
+    cudaStreamSynchronize(s);
+    cudaFree(ell_dev);
+    return e == cudaSuccess ? RTE_OK : RTE_ECUDA;
+}
+
+int rte_media_lognormal(const rte_grid* grid, float dx, uint64_t seed, float mean, float sigma_log, float corr_len,
+                        float* out_dev, float* scratch_dev, void* cuda_stream) {
+    if (!grid || (grid->dim != 2 && grid->dim != 3) || grid->nx < 1 || grid->ny < 1 || grid->nz < 1) return RTE_EINVAL;
+    if (!(dx > 0) || !(mean > 0) || !(sigma_log >= 0) || !(corr_len > 0) || !out_dev || !scratch_dev) return RTE_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const long long G = (long long)grid->nx * grid->ny * grid->nz;
+    const int gb = grid_for(G, 256);
+    double* red = nullptr;
+    if (cudaMalloc((void**)&red, 2 * sizeof(double)) != cudaSuccess) return RTE_ECUDA;
+    cudaMemsetAsync(red, 0, 2 * sizeof(double), s);
+    // kernel std per axis = corr_len/sqrt2 (so the field's covariance is exp(-r^2/(2 corr_len^2)))
+    const float s_cells = corr_len / 1.41421356237f / dx;
+    const int R = (int)std::ceil(4.0f * s_cells);
+    const float inv2s2 = 1.0f / (2.0f * s_cells * s_cells);
+    k_white_noise<<<gb, 256, 0, s>>>(out_dev, G, (unsigned long long)seed);
+    float* a = out_dev;
+    float* b = scratch_dev;
+    for (int axis = 0; axis < grid->dim; ++axis) {
+        k_blur_axis<<<gb, 256, 0, s>>>(b, a, grid->nx, grid->ny, grid->nz, axis, R, inv2s2);
+        float* t = a; a = b; b = t;
+    }
+    if (a != out_dev) cudaMemcpyAsync(out_dev, a, (size_t)G * sizeof(float), cudaMemcpyDeviceToDevice, s);
+    k_moments<<<gb, 256, 0, s>>>(out_dev, G, red);
+    k_lognormal_finish<<<gb, 256, 0, s>>>(out_dev, G, red, mean, sigma_log);
+    cudaError_t e = cudaGetLastError();
+    cudaStreamSynchronize(s);
+    cudaFree(red);
+    return e == cudaSuccess ? RTE_OK : RTE_ECUDA;
+}
+
+int rte_pml_profile(const rte_grid* grid, const rte_pml* pml, float* mu_b_dev, unsigned char* inside_dev,
+                    void* cuda_stream) {
+    if (!grid || !pml || (grid->dim != 2 && grid->dim != 3) || grid->nx < 1 || grid->ny < 1 || grid->nz < 1) return RTE_EINVAL;
+    if (pml->width < 0) return RTE_EINVAL;
+    const long long G = (long long)grid->nx * grid->ny * grid->nz;
+    k_pml_profile<<<grid_for(G, 256), 256, 0, (cudaStream_t)cuda_stream>>>(mu_b_dev, inside_dev, grid->dim, grid->nx,
+                                                                          grid->ny, grid->nz, pml->width, pml->mu_lo,
+                                                                          pml->mu_hi);
+    return cudaGetLastError() == cudaSuccess ? RTE_OK : RTE_ECUDA;
+}
+
+}  // extern "C"

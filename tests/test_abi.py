@@ -1,0 +1,94 @@
+"""Host-side tests of the C-ABI boundary (no GPU): the in-tree library loads, exports every symbol include/rte.h
+declares, validates arguments, and its host-only coefficient tables agree with quadrature and with the oracle."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1801_06364_b200 as rte
+from oracle import rte_oracle as orc
+from test_oracle_pins import quad_coupling
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "rte.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(rte_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_is_in_tree_and_exports_every_declared_symbol():
+    assert os.path.dirname(rte.LIB_PATH) == os.path.join(ROOT, "paper_1801_06364_b200")
+    lib = ctypes.CDLL(rte.LIB_PATH)
+    syms = declared_symbols()
+    assert len(syms) >= 20
+    for s in syms:
+        assert hasattr(lib, s), f"{s} declared in include/rte.h but not exported"
+    assert sorted(rte.EXPORTED) == syms
+
+
+def test_binding_has_same_names():
+    for s in declared_symbols():
+        assert hasattr(rte, s), f"binding lacks {s}"
+
+
+def test_num_coeffs():
+    assert rte.rte_num_coeffs(3, 3) == 16 and rte.rte_num_coeffs(3, 7) == 64 and rte.rte_num_coeffs(3, 5) == 36
+    assert rte.rte_num_coeffs(2, 3) == 7 and rte.rte_num_coeffs(2, 7) == 15
+    assert rte.rte_num_coeffs(4, 3) < 0 and rte.rte_num_coeffs(3, 0) < 0
+
+
+@pytest.mark.parametrize("dim,N", [(3, 1), (3, 2), (3, 3), (3, 5), (3, 7), (2, 1), (2, 3), (2, 7)])
+def test_product_coupling_tables_vs_quadrature_and_oracle(dim, N):
+    """The library's own R7/R8 tables (written in the real basis) vs sphere quadrature and vs the oracle's
+    (complex eq.(10) + change of basis): three independent derivations."""
+    Aq = quad_coupling(dim, N)
+    for axis in range(3):
+        A = rte.rte_coupling_table(dim, N, axis)
+        assert np.abs(A - Aq[axis]).max() < 1e-13
+        Ao, _ = orc.coupling_real(dim, N, axis)
+        assert np.abs(A - Ao).max() < 1e-14
+
+
+def test_workspace_bytes_and_validation():
+    b = rte.rte_workspace_bytes((3, 128, 128, 128), 3)
+    G = 128 ** 3
+    assert b >= 2 * G * 16 * 4 + 3 * G * 4 and b < 2 * G * 16 * 4 + 3 * G * 4 + 5 * 256
+    # 2-D P_3 pads 7 -> 8 fields, P_7 15 -> 16
+    assert rte.rte_workspace_bytes((2, 64, 64, 1), 3) >= 2 * 64 * 64 * 8 * 4
+    with pytest.raises(rte.RteError):
+        rte.rte_workspace_bytes((3, 100, 128, 128), 3)      # unsupported extent
+    with pytest.raises(rte.RteError):
+        rte.rte_workspace_bytes((2, 64, 64, 2), 3)          # nz must be 1 in 2-D
+    with pytest.raises(rte.RteError):
+        rte.rte_workspace_bytes((3, 64, 64, 64), 0)
+
+
+def test_create_fails_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(rte.RteError) as e:
+        rte.rte_create((3, 16, 16, 16), 3, 0.1, 0.001, 0.3, 0.01, 10.0, 0.9)
+    assert e.value.code == rte.RTE_ECUDA
+    # and the raw C entry point reports RTE_ECUDA or RTE_EINVAL, never a silent success
+    lib = ctypes.CDLL(rte.LIB_PATH)
+    out = ctypes.c_void_p()
+    assert lib.rte_create(ctypes.byref(out), None, 3, ctypes.c_float(0.1), ctypes.c_float(0.1), ctypes.c_float(0.3),
+                          None, None, None, 0, None) == rte.RTE_EINVAL
+    assert lib.rte_step(None, 1) == rte.RTE_ESTATE
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1801_06364_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.replace("rte_tables.h, the oracle", "").lower() or f in ("rte_tables.h", "rte_lib.cu"), f
+    for f in ("rte_lib.cu", "rte_pass.cuh", "rte_fft.cuh", "rte_tables.h"):
+        text = open(os.path.join(pkg, "csrc", f)).read()
+        assert "#include \"../../oracle" not in text and "rte_oracle" not in text
