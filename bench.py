@@ -40,7 +40,7 @@ DEFAULT_STEPS = {"cfg0": 2000, "cfg1": 400, "cfg2": 400, "cfg3": 60, "cfg4": 40}
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # bounded oracle sample per workload: (grid extent, PML width, steps) — ~10-30 s of CPU work on ~8-32 cores
 ORACLE_SAMPLE = {"cfg0": (64, 0, 200), "cfg1": (256, 16, 6), "cfg2": (64, 8, 4), "cfg3": (64, 8, 2),
-                 "cfg4": (64, 8, 1)}
+                 "cfg4": (96, 8, 2)}
 
 
 def parse_args(argv=None):
@@ -52,6 +52,7 @@ def parse_args(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
+    ap.add_argument("--no-others", action="store_true", help="skip the short cfg2/cfg3 side measurements")
     a = ap.parse_args(argv)
     if a.steps is None:
         a.steps = DEFAULT_STEPS[a.workload]
@@ -136,3 +137,317 @@ class ClockSampler:
             res.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=smax, reasons=sorted(reasons), samples=len(sm),
                        power_w_max=max(pw) if pw else None)
         return res
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# the oracle legs (the only code in this file that touches oracle/)
+# ---------------------------------------------------------------------------------------------------------------------
+def oracle_sample_config(wl, cfg):
+    n, W, steps = ORACLE_SAMPLE[cfg.name]
+    if n >= max(cfg.nx, cfg.ny, cfg.nz):
+        return cfg, min(steps, cfg.steps), f"{cfg.name} at full size, {min(steps, cfg.steps)} step(s)"
+    small = wl.reduced(cfg, n, pml_width=W)
+    what = f"{cfg.name} structure (P_{cfg.N}, C={cfg.C}) on a {n}^{cfg.dim} grid, PML {small.pml[0]} cells, {steps} step(s)"
+    return small, steps, what
+
+
+def time_oracle(wl, cfg, repeats=1):
+    """Seconds per oracle step on the bounded sample, units (coefficient-cells) per step, threads, description."""
+    import numpy as np
+    from oracle import rte_oracle as orc
+    small, steps, what = oracle_sample_config(wl, cfg)
+    if small.media == "lognormal":      # the CPU generator costs more than the timed steps; a seeded smooth stand-in
+        rng = np.random.default_rng(small.seed)
+        mu = (np.full(small.shape, small.background[0], np.float32),
+              (small.background[1] * np.exp(0.3 * rng.standard_normal(small.shape))).astype(np.float32),
+              np.full(small.shape, small.background[2], np.float32))
+    else:
+        mu = wl.media_maps(small)
+    o = orc.Oracle(small.dim, small.nx, small.ny, small.nz, small.N, small.dx, small.dt, small.c, *mu, *small.pml)
+    o.set_state(wl.random_state(small, seed=1))
+    src = wl.source_term(small)
+    if src is not None:
+        o.set_source(src["w"], src["S"], src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    best = float("inf")
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.step(steps)
+        best = min(best, time.perf_counter() - t0)
+    o.close()
+    return best / steps, small.C * small.G, orc.num_threads(), what
+
+
+def run_reference(args, wl, cfg):
+    """--impl reference: the fp64 oracle on the host cores; one 'step' = one oracle step on the bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    from oracle import rte_oracle as orc
+    small, _, what = oracle_sample_config(wl, cfg)
+    mu = tuple(np.full(small.shape, v, np.float32) for v in small.background) if small.media == "lognormal" \
+        else wl.media_maps(small)
+    o = orc.Oracle(small.dim, small.nx, small.ny, small.nz, small.N, small.dx, small.dt, small.c, *mu, *small.pml)
+    o.set_state(wl.random_state(small, seed=1))
+    src = wl.source_term(small)
+    if src is not None:
+        o.set_source(src["w"], src["S"], src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    if args.warmup:
+        o.step(args.warmup)
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    sec = time.perf_counter() - t0
+    value = small.C * small.G * args.steps / sec
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "sample": what},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": what},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------------------------
+def device_media(rte, wl, cfg, torch, dev):
+    """Media maps generated ON THE DEVICE by the geometry layer (north_star item (3)); scalars for homogeneous."""
+    if cfg.media == "homogeneous":
+        return cfg.background
+    if cfg.media in ("disks", "ellipsoids"):
+        a, s, g = (torch.empty(cfg.shape, dtype=torch.float32, device=dev) for _ in range(3))
+        rte.rte_media_ellipsoids(cfg.grid, cfg.dx, cfg.background, wl.inclusion_list(cfg), a, s, g)
+        return a, s, g
+    if cfg.media == "lognormal":
+        s = torch.empty(cfg.shape, dtype=torch.float32, device=dev)
+        scratch = torch.empty_like(s)
+        rte.rte_media_lognormal(cfg.grid, cfg.dx, cfg.seed, cfg.background[1], cfg.extra["sigma_log"],
+                                cfg.extra["corr_len_mm"], s, scratch)
+        torch.cuda.synchronize()
+        del scratch
+        return cfg.background[0], s, cfg.background[2]
+    raise ValueError(cfg.media)
+
+
+def make_context(rte, wl, cfg, torch, dev):
+    mu_a, mu_s, g = device_media(rte, wl, cfg, torch, dev)
+    ctx = rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, mu_a, mu_s, g, cfg.pml)
+    src = wl.source_term(cfg)
+    if src is not None:
+        rte.rte_set_source(ctx, src["w"], torch.from_numpy(src["S"]).to(dev), src["origin"], src["extent"],
+                           src["kind"], src["t0"], src["sigma_t"])
+    return ctx
+
+
+def device_initial_state(wl, cfg, torch, dev):
+    """psi(0) [C,nz,ny,nx] on the device.  The pulse configs start from their delta / Gaussian initial radiance plus a
+    weak seeded random background (1e-3 of the pulse scale) so that every cell carries non-trivial data; the fields'
+    values do not change the work done."""
+    psi = torch.zeros((cfg.C,) + cfg.shape, dtype=torch.float32, device=dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(cfg.seed)
+    for c in range(cfg.C):
+        psi[c].normal_(0.0, 1e-3, generator=gen)
+    if cfg.source in ("gaussian_pulse_ic", "point_pulse_ic"):
+        cz = cfg.nz // 2 if cfg.dim == 3 else 0
+        if cfg.source == "point_pulse_ic":
+            psi[0, cz, cfg.ny // 2, cfg.nx // 2] += 1.0
+        else:
+            S, org, ext = wl.gaussian_footprint(cfg, (cfg.nx // 2, cfg.ny // 2, cz), cfg.extra["sigma_mm"])
+            psi[0, org[2]:org[2] + ext[2], org[1]:org[1] + ext[1], org[0]:org[0] + ext[0]] += \
+                torch.from_numpy(S).to(dev) * (cfg.dx ** cfg.dim)
+    return psi
+
+
+def timed_steps(rte, ctx, torch, steps, dist=None):
+    """K steps bracketed by barrier + synchronize on both sides; device time by CUDA events on the launch stream."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    rte.rte_step(ctx, steps)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return e0.elapsed_time(e1)
+
+
+def measure_workload(rte, wl, cfg, torch, dev, steps, warmup, dist=None, sampler=None):
+    """Device-resident throughput + per-axis kernel times for one workload.  Returns a dict."""
+    ctx = make_context(rte, wl, cfg, torch, dev)
+    psi0 = device_initial_state(wl, cfg, torch, dev)
+    rte.rte_set_state(ctx, psi0)
+    del psi0
+    rte.rte_step(ctx, warmup)
+    rte.rte_sync(ctx)
+    l0 = rte.rte_launch_count(ctx)
+    if sampler is not None:
+        sampler.start()
+    ms = timed_steps(rte, ctx, torch, steps, dist)
+    clocks = sampler.stop() if sampler is not None else None
+    launches = rte.rte_launch_count(ctx) - l0
+    # per-kernel times, measured live with CUDA events on the context's stream (same launch configuration)
+    nprof = max(3, min(steps, 20))
+    ms_axis, n_axis = rte.rte_step_profile(ctx, nprof)
+    phi = torch.empty(cfg.shape, dtype=torch.float32, device=dev)
+    rte.rte_fluence(ctx, phi)
+    rte.rte_sync(ctx)
+    finite = bool(torch.isfinite(phi).all().item())
+    return dict(ctx=ctx, ms=ms, launches=launches, clocks=clocks, finite=finite,
+                ms_axis=[m / max(1, n) for m, n in zip(ms_axis, n_axis)], prof_steps=nprof)
+
+
+def roofline_of(cfg, res, peak, peak_kind):
+    per_axis, per_step = algorithmic_bytes(cfg)
+    naxes = cfg.dim
+    names = ["pass_x (DFT-ik-IDFT + coupling, first)", "pass_y (middle, accumulates)", "pass_z (last: + sigma_l, PML, source, Euler)"]
+    if cfg.dim == 2:
+        names = [names[0], "pass_y (last: + sigma_l, PML, source, Euler)", ""]
+    dom = max(range(naxes), key=lambda a: res["ms_axis"][a])
+    ach = per_axis[dom] / (res["ms_axis"][dom] * 1e-3) / 1e9
+    kernels = []
+    for a in range(naxes):
+        gbs = per_axis[a] / (res["ms_axis"][a] * 1e-3) / 1e9
+        kernels.append({"kernel": names[a], "ms": res["ms_axis"][a], "algorithmic_bytes": per_axis[a],
+                        "achieved_gbs": gbs, "frac": gbs / peak})
+    step_gbs = per_step / (1e-3 * sum(res["ms_axis"][:naxes])) / 1e9
+    return {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "peak_kind": peak_kind + " (burst copy)",
+            "unit": "GB/s", "frac": ach / peak, "traffic": TRAFFIC_NCU.get(cfg.name, {}).get(dom),
+            "bytes_per_coefficient_cell_step": per_step / (cfg.C * cfg.G),
+            "whole_step": {"algorithmic_bytes": per_step, "achieved_gbs": step_gbs, "frac": step_gbs / peak,
+                           "frac_of_nominal_8000": step_gbs / 8000.0},
+            "kernels": kernels}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
+# captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
+TRAFFIC_NCU = {}
+
+
+def run_ours(args, wl, cfg):
+    import torch
+    try:
+        import paper_1801_06364_b200 as rte
+    except ImportError as e:     # fail loudly: there is no fallback path
+        print(f"bench.py: the CUDA library is not built: {e}", file=sys.stderr)
+        return 2
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; this path has no CPU fallback", file=sys.stderr)
+        return 2
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=dev)
+        dist = dist_mod
+    peak, peak_kind = hbm_peak()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    res = measure_workload(rte, wl, cfg, torch, dev, args.steps, args.warmup, dist, sampler)
+    ms = res["ms"]
+    if dist is not None:      # max over ranks of the device time
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    units = cfg.C * cfg.G * args.steps * world
+    value = units / (ms * 1e-3)
+    ctx = res["ctx"]
+
+    # ---- e2e: host buffers through the C ABI (pinned host -> device state, K steps, fluence device -> host) ----------
+    e2e = None
+    if not args.no_e2e:
+        h_state = torch.empty((cfg.C,) + cfg.shape, dtype=torch.float32, pin_memory=True)
+        rte.rte_get_state_host(ctx, h_state)            # a real state to upload
+        h_phi = torch.empty(cfg.shape, dtype=torch.float32, pin_memory=True)
+        rte.rte_set_state_host(ctx, h_state)            # warm the path once
+        rte.rte_step(ctx, 1)
+        rte.rte_fluence_host(ctx, h_phi)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        rte.rte_set_state_host(ctx, h_state)
+        rte.rte_step(ctx, args.steps)
+        rte.rte_fluence_host(ctx, h_phi)                # synchronises the stream
+        e1.record()
+        torch.cuda.synchronize()
+        wall_ms = 1e3 * (time.perf_counter() - t0)
+        e_ms = max(e0.elapsed_time(e1), wall_ms)
+        if dist is not None:
+            t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": units / (e_ms * 1e-3), "unit": UNIT, "ms_total": e_ms,
+               "h2d_bytes_per_step": h_state.numel() * 4 / args.steps, "d2h_bytes_per_step": h_phi.numel() * 4 / args.steps,
+               "what": f"rte_set_state_host (pinned, {h_state.numel() * 4 / 1e9:.2f} GB) + {args.steps} x rte_step + rte_fluence_host, per rank"}
+        del h_state, h_phi
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    roof = roofline_of(cfg, res, peak, peak_kind)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz][:cfg.dim], "P_N": cfg.N, "coefficients": cfg.C,
+                       "cells": cfg.G, "state_bytes": 4 * cfg.C * cfg.G, "dx_mm": cfg.dx, "dt_ps": cfg.dt,
+                       "pml_cells": cfg.pml[0], "media": cfg.media, "source": cfg.source,
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "state larger than L2 (no flush needed)" if 4 * cfg.C * cfg.G > 2 * 126e6
+                             else "state comparable to / smaller than the 126 MB L2: DRAM fraction not meaningful"},
+            "clocks": res["clocks"], "e2e": e2e, "gpu_launches": res["launches"], "finite": res["finite"],
+            "roofline": roof,
+            "paper_context": {"k40_updates_per_s_complex": [7.25e8, 1.88e9], "source": "PAPER.md:141,167 (Tesla K40; context only)"}}
+
+    if not args.no_others and world == 1 and cfg.name == DEFAULT_WORKLOAD:
+        del res, ctx
+        torch.cuda.empty_cache()
+        others = {}
+        for name in ("cfg2", "cfg3"):
+            c2 = wl.CONFIGS[name]
+            r2 = measure_workload(rte, wl, c2, torch, dev, DEFAULT_STEPS[name], max(3, args.warmup))
+            rf = roofline_of(c2, r2, peak, peak_kind)
+            others[name] = {"ms_per_step": r2["ms"] / DEFAULT_STEPS[name],
+                            "value": c2.C * c2.G * DEFAULT_STEPS[name] / (r2["ms"] * 1e-3),
+                            "whole_step_frac": rf["whole_step"]["frac"], "dominant_kernel_frac": rf["frac"],
+                            "finite": r2["finite"]}
+            del r2
+            torch.cuda.empty_cache()
+        line["other_3d_workloads"] = others
+
+    if not args.no_cpu_baseline:
+        sec, units_small, cores, what = time_oracle(wl, cfg)
+        line["cpu_baseline"] = {"value": units_small / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "ms_per_step": 1e3 * sec, "sample": what}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    import rte_workloads as wl
+    cfg = wl.CONFIGS[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, wl, cfg)
+    return run_ours(args, wl, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
