@@ -28,8 +28,7 @@ struct AxisTables {
     float2* tw = nullptr;
     float* kap = nullptr;
     CplEntry* cpl = nullptr;
-    int* cpl_cnt = nullptr;
-    int n = 0, N1 = 0, N2 = 0;
+    int n = 0, N1 = 0, N2 = 0, maxcnt = 0;
 };
 
 }  // namespace
@@ -349,64 +348,108 @@ int check_grid(const rte_grid* g) {
 // ---------------------------------------------------------------------------------------------------------------------
 // pass dispatch
 // ---------------------------------------------------------------------------------------------------------------------
-struct LaunchPlan { int TP, nt, blocks; size_t smem; };
+// A pass runs either a kernel specialised at compile time for (n, P, TP, block size) — the five BASELINE.json
+// configurations — or the generic kernel (run-time P, TP, block size) for every other supported extent / order.
+struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; };
+
+struct SpecRow { int n, P, TP, nt; };
+constexpr SpecRow kSpec[] = {
+    {384, 32, 1, 256},   // cfg4: 384^3 P_7   (98 KB tile, 2 CTAs / SM)
+    {256, 18, 2, 288},   // cfg3: 256^3 P_5   (288 B chunks = 9 whole sectors)
+    {128, 8, 4, 256},    // cfg2: 128^3 P_3
+    {512, 8, 2, 256},    // cfg1: 512^2 P_7 (2-D)
+    {64, 4, 8, 256},     // cfg0: 64^2 P_3 (2-D)
+};
+
+size_t pass_smem(int n, int Q, int TP, int nsig, bool first) {
+    size_t b = (size_t)n * Q * sizeof(float2) + (size_t)n * sizeof(float2) + (size_t)n * sizeof(float);
+    if (first) b += (size_t)nsig * ((size_t)n * TP + 1) * sizeof(float);
+    return b;
+}
+
+constexpr size_t kMaxSmem = 227 * 1024;
 
 LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz;
     int groups = 1;
     if (axis == 0) { A.stride_i = 1; A.stride_t = nx; A.group_stride = 0; A.pencils_per_group = ny * nz; }
     else if (axis == 1) {
-        A.stride_i = nx; A.stride_t = 1; A.group_stride = nx * ny; A.pencils_per_group = nx; groups = nz;
+        A.stride_i = nx; A.stride_t = 1; A.group_stride = (long long)nx * ny; A.pencils_per_group = nx; groups = nz;
     } else { A.stride_i = nx * ny; A.stride_t = 1; A.group_stride = 0; A.pencils_per_group = nx * ny; }
     const AxisTables& T = c->ax[axis];
     const int P = c->P, n = T.n;
-    int tp = 1;
-    while (tp * P < 32 && tp < 8) tp *= 2;
-    while (tp > 1 && (size_t)n * tp * P * 8 > 96 * 1024) tp /= 2;
-    while (tp > 1 && tp > A.pencils_per_group) tp /= 2;
-    A.TP = tp; A.P = P;
-    A.tiles_per_group = (A.pencils_per_group + tp - 1) / tp;
-    const int Q = tp * P;
-    const int T1 = Q * T.N2, T2 = Q * T.N1;
-    int best = 128; double best_cost = 1e30;
-    for (int nt = 64; nt <= 320; nt += 32) {
-        if (nt > T1 && nt > T2 && nt > 64) break;
-        const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;
-        const double cost = w1 + w2;
-        if (cost <= best_cost + 1e-12) { best_cost = cost; best = nt; }
+    const bool first = axis == 0;
+    LaunchPlan L{};
+    L.spec = -1;
+    A.P = P;
+    for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
+        if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
+            !(axis == c->grid.dim - 1 && c->grid.dim == 3 && T.maxcnt > 3)) {
+            L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
+            break;
+        }
+    if (L.spec < 0) {
+        int tp = 1;
+        while (tp * P < 32 && tp < 8) tp *= 2;
+        while (tp > 1 && pass_smem(n, tp * P, tp, c->N + 1, first) > 100 * 1024) tp /= 2;
+        while (tp > 1 && tp > A.pencils_per_group) tp /= 2;
+        const int Q = tp * P;
+        const int T1 = Q * T.N2, T2 = Q * T.N1;
+        int best = 128; double best_cost = 1e30;
+        for (int nt = 64; nt <= 320; nt += 32) {
+            if (nt > T1 && nt > T2 && nt > 64) break;
+            const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;
+            const double cost = w1 + w2;
+            if (cost <= best_cost + 1e-12) { best_cost = cost; best = nt; }
+        }
+        L.TP = tp; L.nt = best;
     }
-    LaunchPlan L;
-    L.TP = tp; L.nt = best; L.blocks = groups * A.tiles_per_group;
-    L.smem = (size_t)n * Q * sizeof(float2) + (size_t)n * sizeof(float2) + (size_t)n * sizeof(float);
+    A.TP = L.TP;
+    A.tiles_per_group = (A.pencils_per_group + L.TP - 1) / L.TP;
+    L.blocks = groups * A.tiles_per_group;
+    L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, first);
     return L;
 }
 
-template <int N1, int N2, int MODE>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
-    auto kern = rtepass::pass_kernel<N1, N2, MODE>;
-    static size_t configured = 0;
-    if (L.smem > 48 * 1024 && L.smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200 * 1024));
+    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
         if (e != cudaSuccess) return e;
-        configured = 200 * 1024;
+        configured = true;
     }
     kern<<<L.blocks, L.nt, L.smem, s>>>(A);
     return cudaGetLastError();
 }
 
 template <int MODE>
-cudaError_t launch_mode(int n, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
+cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     switch (n) {
-        case 16: return launch_one<4, 4, MODE>(A, L, s);
-        case 32: return launch_one<4, 8, MODE>(A, L, s);
-        case 48: return launch_one<4, 12, MODE>(A, L, s);
-        case 64: return launch_one<8, 8, MODE>(A, L, s);
-        case 96: return launch_one<8, 12, MODE>(A, L, s);
-        case 128: return launch_one<8, 16, MODE>(A, L, s);
-        case 192: return launch_one<12, 16, MODE>(A, L, s);
-        case 256: return launch_one<16, 16, MODE>(A, L, s);
-        case 384: return launch_one<24, 16, MODE>(A, L, s);
-        case 512: return launch_one<32, 16, MODE>(A, L, s);
+        case 16: return launch_one<4, 4, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 32: return launch_one<4, 8, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 48: return launch_one<4, 12, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 64: return launch_one<8, 8, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 96: return launch_one<8, 12, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 128: return launch_one<8, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 192: return launch_one<12, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 256: return launch_one<16, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 384: return launch_one<24, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        case 512: return launch_one<32, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+// E = 3 on the z axis of 3-D runs (fan-in of the z coupling is at most 3 pairs), 4 otherwise
+template <int MODE, int E>
+cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
+    switch (spec) {
+        case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2>(A, L, s);
+        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, 2>(A, L, s);
+        case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, 3>(A, L, s);
+        case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2>(A, L, s);
+        case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3>(A, L, s);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -421,23 +464,31 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
     const int naxes = c->grid.dim;
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
-        A.psi = c->psi; A.part = c->part; A.out = c->psi;
-        A.tw = c->ax[axis].tw; A.kap = c->ax[axis].kap; A.cpl = c->ax[axis].cpl; A.cpl_cnt = c->ax[axis].cpl_cnt;
+        A.psi = c->psi; A.acc = c->part; A.out = c->psi;
+        A.tw = c->ax[axis].tw; A.kap = c->ax[axis].kap; A.cpl = c->ax[axis].cpl;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
-        A.cdt = c->c * c->dt;
+        A.cdt = c->c * c->dt; A.nsig = c->N + 1;
         A.srcS = c->srcS; A.srcw = c->srcw;
         for (int k = 0; k < 3; ++k) { A.src_org[k] = c->src_org[k]; A.src_ext[k] = c->src_ext[k]; }
         A.src_amp = 0.f;
         A.nx = c->grid.nx; A.ny = c->grid.ny;
         const LaunchPlan L = plan_pass(c, axis, A);
-        const int mode = axis == 0 ? rtepass::MODE_FIRST : (axis == naxes - 1 ? rtepass::MODE_LAST : rtepass::MODE_MIDDLE);
+        const int n = c->ax[axis].n;
         cudaError_t e;
-        if (mode == rtepass::MODE_LAST) {
+        if (axis == 0) {
             if (c->src_kind != 0)
                 A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, (double)c->steps * (double)c->dt));
-            e = launch_mode<rtepass::MODE_LAST>(c->ax[axis].n, A, L, c->stream);
-        } else if (mode == rtepass::MODE_FIRST) e = launch_mode<rtepass::MODE_FIRST>(c->ax[axis].n, A, L, c->stream);
-        else e = launch_mode<rtepass::MODE_MIDDLE>(c->ax[axis].n, A, L, c->stream);
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream)
+                            : launch_generic<rtepass::MODE_FIRST>(n, A, L, c->stream);
+        } else if (axis == naxes - 1) {
+            if (L.spec >= 0)
+                e = naxes == 3 ? launch_spec<rtepass::MODE_LAST, 3>(L.spec, A, L, c->stream)
+                               : launch_spec<rtepass::MODE_LAST, 4>(L.spec, A, L, c->stream);
+            else e = launch_generic<rtepass::MODE_LAST>(n, A, L, c->stream);
+        } else {
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_MIDDLE, 4>(L.spec, A, L, c->stream)
+                            : launch_generic<rtepass::MODE_MIDDLE>(n, A, L, c->stream);
+        }
         if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
         c->launches += 1;
         if (ev) cudaEventRecord(ev[axis], c->stream);
@@ -458,7 +509,7 @@ cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t s) {
 void free_ctx(rte_ctx* c) {
     if (!c) return;
     for (int a = 0; a < 3; ++a) {
-        cudaFree(c->ax[a].tw); cudaFree(c->ax[a].kap); cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_cnt);
+        cudaFree(c->ax[a].tw); cudaFree(c->ax[a].kap); cudaFree(c->ax[a].cpl);
     }
     cudaFree(c->deg); cudaFree(c->ext_of_slot); cudaFree(c->srcw); cudaFree(c->srcS); cudaFree(c->phi_prev);
     cudaFree(c->red);
@@ -579,6 +630,22 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
     ctx->ss = (float*)w; w += map;
     ctx->gm = (float*)w;
 
+    // every pass tile (one pencil of all pairs + tables) must fit in shared memory, and the byte stride between the
+    // N1 cells a thread touches must fit 32 bits (rte_pass.cuh byte_off)
+    {
+        const int ext[3] = {grid->nx, grid->ny, grid->nz};
+        const long long str[3] = {1, grid->nx, (long long)grid->nx * grid->ny};
+        for (int a = 0; a < grid->dim; ++a) {
+            int n1 = 0, n2 = 0;
+            rtetab::split_of(ext[a], n1, n2);
+            if (pass_smem(ext[a], ctx->P, 1, N + 1, a == 0) > kMaxSmem ||
+                (unsigned long long)32 * (unsigned long long)str[a] * (unsigned long long)ctx->P * 8ull >= (1ull << 32)) {
+                delete ctx;
+                return fail(nullptr, RTE_EUNSUPPORTED, "grid extent x number of coefficients exceeds one shared-memory pencil tile");
+            }
+        }
+    }
+
 #define CREATE_TRY(expr)                                                                         \
     do {                                                                                         \
         cudaError_t e__ = (expr);                                                                \
@@ -604,19 +671,24 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
         CREATE_TRY(upload(&T.kap, kap, ctx->stream));
         std::vector<std::vector<rtetab::PairEntry>> pe;
         rtetab::pair_coupling(grid->dim, N, a, pe);
-        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE, CplEntry{0, 0.f, 0.f, 0.f, 0.f});
-        std::vector<int> cnt(ctx->P, 0);
+        // weights pre-multiplied by -c dt (eq.(11)); unused entries point at the pair itself with zero weights
+        const double mcdt = -(double)c * (double)dt;
+        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE);
+        T.maxcnt = 0;
         for (int p = 0; p < ctx->P; ++p) {
-            if ((int)pe[p].size() > rtepass::kMaxE) {
+            const int cnt = (int)pe[p].size();
+            if (cnt > rtepass::kMaxE) {
                 free_ctx(ctx);
                 return fail(nullptr, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
             }
-            cnt[p] = (int)pe[p].size();
-            for (int e = 0; e < cnt[p]; ++e)
-                flat[(size_t)p * rtepass::kMaxE + e] = CplEntry{pe[p][e].src, pe[p][e].w00, pe[p][e].w01, pe[p][e].w10, pe[p][e].w11};
+            if (cnt > T.maxcnt) T.maxcnt = cnt;
+            for (int e = 0; e < rtepass::kMaxE; ++e)
+                flat[(size_t)p * rtepass::kMaxE + e] =
+                    e < cnt ? CplEntry{pe[p][e].src, (float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w01),
+                                       (float)(mcdt * pe[p][e].w10), (float)(mcdt * pe[p][e].w11)}
+                            : CplEntry{p, 0.f, 0.f, 0.f, 0.f};
         }
         CREATE_TRY(upload(&T.cpl, flat, ctx->stream));
-        CREATE_TRY(upload(&T.cpl_cnt, cnt, ctx->stream));
     }
     {
         std::vector<int> eos, deg;
