@@ -46,13 +46,54 @@ __host__ __device__ constexpr double sin2pi(int num, int den) {    // sin(2 pi x
     return cos2pi(4 * num - den, 4 * den);
 }
 
-RTE_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-RTE_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-RTE_HD float2 cmul(float2 a, float2 w) {   // a * w
-    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.y, w.x, a.x * w.y));
+// ---- packed complex arithmetic ----------------------------------------------------------------------------------------
+// A complex number is one float2 = one aligned 64-bit register pair.  sm_100a has packed fp32 instructions
+// (PTX add/mul/fma.rn.f32x2 -> SASS FADD2/FMUL2/FFMA2) that do both halves in ONE issue slot, and ptxas folds the
+// half-swap, the per-half negation and the scalar broadcast of the operands below into operand modifiers
+// (.LO_HI, .NP, .F32), so a complex add is 1 instruction and a complex-by-constant multiply is 2 (scalar: 2 and 4).
+// Same IEEE roundings as the scalar forms (each half is an independent fp32 add / mul / fma).
+#ifdef __CUDA_ARCH__
+typedef unsigned long long c64_t;
+__device__ __forceinline__ c64_t pk(float lo, float hi) { c64_t r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float2 up(c64_t v) { float2 r; asm("mov.b64 {%0,%1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r; }
+__device__ __forceinline__ c64_t add2(c64_t a, c64_t b) { c64_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ c64_t mul2(c64_t a, c64_t b) { c64_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ c64_t fma2(c64_t a, c64_t b, c64_t c) { c64_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+#define RTE_PACKED(packed_expr, scalar_expr) return packed_expr
+#else
+#define RTE_PACKED(packed_expr, scalar_expr) return scalar_expr
+#endif
+RTE_HD float2 cadd(float2 a, float2 b) { RTE_PACKED(up(add2(pk(a.x, a.y), pk(b.x, b.y))), make_float2(a.x + b.x, a.y + b.y)); }
+RTE_HD float2 csub(float2 a, float2 b) { RTE_PACKED(up(add2(pk(a.x, a.y), pk(-b.x, -b.y))), make_float2(a.x - b.x, a.y - b.y)); }
+RTE_HD float2 cadd_mi(float2 a, float2 b) {   // a - i b
+    RTE_PACKED(up(add2(pk(a.x, a.y), pk(b.y, -b.x))), make_float2(a.x + b.y, a.y - b.x));
 }
-RTE_HD float2 cmulc(float2 a, float2 w) {  // a * conj(w)
-    return make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(-a.x, w.y, a.y * w.x));
+RTE_HD float2 cadd_pi(float2 a, float2 b) {   // a + i b
+    RTE_PACKED(up(add2(pk(a.x, a.y), pk(-b.y, b.x))), make_float2(a.x - b.y, a.y + b.x));
+}
+RTE_HD float2 cscale(float2 a, float s) { RTE_PACKED(up(mul2(pk(a.x, a.y), pk(s, s))), make_float2(a.x * s, a.y * s)); }
+RTE_HD float2 cmul_cs(float2 a, float c, float s) {   // a * (c - i s) = c (a.x, a.y) + s (a.y, -a.x)
+    RTE_PACKED(up(fma2(pk(a.y, -a.x), pk(s, s), mul2(pk(a.x, a.y), pk(c, c)))),
+               make_float2(fmaf(a.y, s, a.x * c), fmaf(-a.x, s, a.y * c)));
+}
+RTE_HD float2 cmul(float2 a, float2 w) {   // a * w = w.x (a.x, a.y) + w.y (-a.y, a.x)
+    RTE_PACKED(up(fma2(pk(-a.y, a.x), pk(w.y, w.y), mul2(pk(a.x, a.y), pk(w.x, w.x)))),
+               make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x)));
+}
+RTE_HD float2 cmulc(float2 a, float2 w) {  // a * conj(w) = w.x (a.x, a.y) + w.y (a.y, -a.x)
+    RTE_PACKED(up(fma2(pk(a.y, -a.x), pk(w.y, w.y), mul2(pk(a.x, a.y), pk(w.x, w.x)))),
+               make_float2(fmaf(a.y, w.y, a.x * w.x), fmaf(-a.x, w.y, a.y * w.x)));
+}
+RTE_HD float2 caxpy(float s, float2 a, float2 acc) {   // acc + s * a (both halves)
+    RTE_PACKED(up(fma2(pk(s, s), pk(a.x, a.y), pk(acc.x, acc.y))), make_float2(fmaf(s, a.x, acc.x), fmaf(s, a.y, acc.y)));
+}
+// acc + (wx * a.x, wy * a.y): the diagonal part of a 2x2 real block applied to a pair
+RTE_HD float2 cfma_diag(float wx, float wy, float2 a, float2 acc) {
+    RTE_PACKED(up(fma2(pk(wx, wy), pk(a.x, a.y), pk(acc.x, acc.y))), make_float2(fmaf(wx, a.x, acc.x), fmaf(wy, a.y, acc.y)));
+}
+// acc + (wx * a.y, wy * a.x): the off-diagonal part
+RTE_HD float2 cfma_swap(float wx, float wy, float2 a, float2 acc) {
+    RTE_PACKED(up(fma2(pk(wx, wy), pk(a.y, a.x), pk(acc.x, acc.y))), make_float2(fmaf(wx, a.y, acc.x), fmaf(wy, a.x, acc.y)));
 }
 
 // a * exp(-2 pi i NUM/DEN) with the multiples of an eighth turn special-cased
@@ -64,14 +105,14 @@ RTE_HD float2 mulw(float2 a) {
     else if constexpr (4 * r == DEN) return make_float2(a.y, -a.x);                       // * -i
     else if constexpr (2 * r == DEN) return make_float2(-a.x, -a.y);                      // * -1
     else if constexpr (4 * r == 3 * DEN) return make_float2(-a.y, a.x);                   // * +i
-    else if constexpr (8 * r == DEN) return make_float2((a.x + a.y) * h, (a.y - a.x) * h);        // (1-i)/sqrt2
-    else if constexpr (8 * r == 3 * DEN) return make_float2((a.y - a.x) * h, -(a.x + a.y) * h);   // (-1-i)/sqrt2
-    else if constexpr (8 * r == 5 * DEN) return make_float2(-(a.x + a.y) * h, (a.x - a.y) * h);   // (-1+i)/sqrt2
-    else if constexpr (8 * r == 7 * DEN) return make_float2((a.x - a.y) * h, (a.x + a.y) * h);    // (1+i)/sqrt2
+    else if constexpr (8 * r == DEN) return cscale(cadd_mi(a, a), h);                     // (1-i)/sqrt2:  h (a - i a)
+    else if constexpr (8 * r == 3 * DEN) return cscale(cadd_pi(a, a), -h);                // (-1-i)/sqrt2: -h (a + i a)
+    else if constexpr (8 * r == 5 * DEN) return cscale(cadd_mi(a, a), -h);                // (-1+i)/sqrt2: -h (a - i a)
+    else if constexpr (8 * r == 7 * DEN) return cscale(cadd_pi(a, a), h);                 // (1+i)/sqrt2:  h (a + i a)
     else {
         constexpr float c = (float)cos2pi(r, DEN);
         constexpr float s = (float)sin2pi(r, DEN);   // w = c - i s
-        return make_float2(fmaf(a.y, s, a.x * c), fmaf(-a.x, s, a.y * c));
+        return cmul_cs(a, c, s);
     }
 }
 
@@ -99,11 +140,11 @@ struct Dft<3, S> {
         constexpr float hs3 = 0.86602540378443864676f;   // sqrt(3)/2
         const float2 a = v[0], b = v[S], c = v[2 * S];
         const float2 s = cadd(b, c), d = csub(b, c);
-        const float2 m = make_float2(fmaf(-0.5f, s.x, a.x), fmaf(-0.5f, s.y, a.y));
+        const float2 m = caxpy(-0.5f, s, a);
         // X1 = m - i hs3 d ; X2 = m + i hs3 d
         v[0] = cadd(a, s);
-        v[S] = make_float2(fmaf(hs3, d.y, m.x), fmaf(-hs3, d.x, m.y));
-        v[2 * S] = make_float2(fmaf(-hs3, d.y, m.x), fmaf(hs3, d.x, m.y));
+        v[S] = caxpy(hs3, make_float2(d.y, -d.x), m);
+        v[2 * S] = caxpy(hs3, make_float2(-d.y, d.x), m);
     }
 };
 
@@ -114,8 +155,8 @@ struct Dft<4, S> {
         const float2 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = csub(b, d);
         v[0] = cadd(t0, t2);
         v[2 * S] = csub(t0, t2);
-        v[S] = make_float2(t1.x + t3.y, t1.y - t3.x);       // t1 - i t3
-        v[3 * S] = make_float2(t1.x - t3.y, t1.y + t3.x);   // t1 + i t3
+        v[S] = cadd_mi(t1, t3);       // t1 - i t3
+        v[3 * S] = cadd_pi(t1, t3);   // t1 + i t3
     }
 };
 

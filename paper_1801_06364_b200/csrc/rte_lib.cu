@@ -367,7 +367,7 @@ size_t pass_smem(int n, int Q, int TP, int nsig, bool first) {
     return b;
 }
 
-constexpr size_t kMaxSmem = 227 * 1024;
+constexpr size_t kMaxSmem = 226 * 1024;   // 227 KB per CTA minus the static mbarrier slot
 
 LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz;
@@ -408,6 +408,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     A.tiles_per_group = (A.pencils_per_group + L.TP - 1) / L.TP;
     L.blocks = groups * A.tiles_per_group;
     L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, first);
+    if (L.spec >= 0 && first && L.TP > 1) L.smem += (size_t)L.TP * (P % 16) * sizeof(float2);   // stacked-layout padding
     return L;
 }
 
@@ -684,9 +685,9 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
             if (cnt > T.maxcnt) T.maxcnt = cnt;
             for (int e = 0; e < rtepass::kMaxE; ++e)
                 flat[(size_t)p * rtepass::kMaxE + e] =
-                    e < cnt ? CplEntry{pe[p][e].src, (float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w01),
-                                       (float)(mcdt * pe[p][e].w10), (float)(mcdt * pe[p][e].w11)}
-                            : CplEntry{p, 0.f, 0.f, 0.f, 0.f};
+                    e < cnt ? CplEntry{(float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w11),
+                                       (float)(mcdt * pe[p][e].w01), (float)(mcdt * pe[p][e].w10), pe[p][e].src, 0}
+                            : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
         }
         CREATE_TRY(upload(&T.cpl, flat, ctx->stream));
     }

@@ -17,7 +17,12 @@
 // axis is a sequence of P*8-byte contiguous chunks and one complex FFT differentiates two real fields.
 //
 // Index conventions inside a tile: i = position along the pencil (0..n-1), t = pencil within the tile (0..TP-1),
-// p = pair (0..P-1), q = t*P + p (0..Q-1).  Shared tile: tile[i*Q + q].  n = N1*N2, i = a*N2 + b, k = k1 + N1*k2.
+// p = pair (0..P-1), q = t*P + p (0..Q-1).  n = N1*N2, i = a*N2 + b, k = k1 + N1*k2.
+// Shared tile: element (i, t, p) lives at tile[i*SI + t*ST + p] with
+//   (SI, ST) = (Q, P)             "interleaved": y/z passes and every generic kernel — the global order of a y/z tile
+//   (SI, ST) = (P, n*P + pad)     "stacked":     x pass of the specialised kernels — the global order of an x tile
+// so that the specialised kernels fill the tile with a few TMA bulk copies (cp.async.bulk, SASS UBLKCP) that complete
+// on an mbarrier while the CTA loads its tables; the generic kernels load through registers.
 // QC / PC / NTC are compile-time copies of Q, P and the block size (0 = run-time value) so that every shared-memory
 // offset of the unrolled transforms folds into an instruction immediate for the configurations that matter.
 #pragma once
@@ -27,7 +32,10 @@ namespace rtepass {
 
 constexpr int kMaxE = 4;   // max source pairs per output pair and axis (checked on the host when tables are built)
 
-struct CplEntry { int src; float w00, w01, w10, w11; };   // weights already multiplied by -c dt
+// One 2x2 real block of the coupling: T.x += wd0 d.x + ws0 d.y ; T.y += wd1 d.y + ws1 d.x  (wd = diagonal (w00, w11),
+// ws = off-diagonal (w01, w10); stored as the two register pairs of the packed FFMA2 form).  Weights already
+// multiplied by -c dt.
+struct alignas(8) CplEntry { float wd0, wd1, ws0, ws1; int src; int pad_; };
 
 enum { MODE_FIRST = 0, MODE_MIDDLE = 1, MODE_LAST = 2 };
 
@@ -62,83 +70,165 @@ struct PassArgs {
 
 #ifdef __CUDACC__
 
-template <typename T>
-__device__ __forceinline__ T* byte_off(T* p, unsigned stepB, int a) {
-    // p + a*stepB bytes: one IMAD.WIDE.U32 with the 64-bit base as addend (a is a compile-time constant at all uses)
-    return reinterpret_cast<T*>(reinterpret_cast<uintptr_t>(p) + (unsigned long long)stepB * (unsigned)a);
+// ---- global memory access with explicit state space (keeps LDG/STG instead of generic LD/ST after byte offsets) ------
+__device__ __forceinline__ float2 ldg64(const float2* p, unsigned long long byte_offset) {
+    float2 v;
+    asm volatile("ld.global.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(reinterpret_cast<const char*>(p) + byte_offset));
+    return v;
+}
+__device__ __forceinline__ void stg64(float2* p, unsigned long long byte_offset, float2 v) {
+    asm volatile("st.global.v2.f32 [%0], {%1,%2};" ::"l"(reinterpret_cast<char*>(p) + byte_offset), "f"(v.x), "f"(v.y) : "memory");
 }
 
-// ---- phase 1: HBM -> registers, first factor forward, -> shared -----------------------------------------------------
-template <int N1, int N2, int QC, int PC>
+// ---- mbarrier + TMA bulk copy (global -> shared) ----------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- tile geometry ------------------------------------------------------------------------------------------------------
+// STACKED (x pass of a specialised kernel): tile[(t*(n*P + pad) + i*P + p]; otherwise tile[i*Q + t*P + p].
+// pad = P mod 16 float2 keeps the lanes of a half-warp (consecutive p, then the next pencil) on distinct banks.
+template <int N1, int N2, int QC, int PC, bool STACKED>
+struct Geo {
+    static constexpr int n = N1 * N2;
+    static constexpr int TPC = QC / (PC ? PC : 1);
+    static constexpr int pad = (STACKED && TPC > 1) ? (PC % 16) : 0;
+    static constexpr int SI = STACKED ? PC : QC;             // 0 when run-time
+    static constexpr int ST = STACKED ? n * PC + pad : PC;
+    static constexpr int tile_elems = STACKED ? TPC * ST : n * QC;
+};
+
+// ---- phase 0 (specialised kernels): the whole psi tile by TMA bulk copies ------------------------------------------------
+template <int N1, int N2, int QC, int PC, bool STACKED>
+__device__ __forceinline__ void tile_tma_load(const PassArgs& A, float2* tile, long long base, unsigned long long* bar, int tid,
+                                              int nt) {
+    using G = Geo<N1, N2, QC, PC, STACKED>;
+    if (STACKED) {
+        // TP whole pencils of n*P*8 contiguous bytes each, issued as 16 KB pieces by different threads
+        constexpr unsigned pen_bytes = (unsigned)G::n * PC * 8u;
+        constexpr unsigned piece = pen_bytes % 16384u == 0 ? 16384u : (pen_bytes % 4096u == 0 ? 4096u : pen_bytes);
+        constexpr int pieces = (int)(pen_bytes / piece);
+        for (int j = tid; j < G::TPC * pieces; j += nt) {
+            const int t = j / pieces, k = j - t * pieces;
+            const char* src = reinterpret_cast<const char*>(A.psi + (base + (long long)t * A.stride_t) * PC) + (size_t)k * piece;
+            char* dst = reinterpret_cast<char*>(tile + t * G::ST) + (size_t)k * piece;
+            tma_load_1d(dst, src, piece, bar);
+        }
+    } else {
+        // n rows of Q*8 contiguous bytes (neighbouring pencils of a y/z tile are neighbouring cells)
+        for (int i = tid; i < G::n; i += nt)
+            tma_load_1d(tile + i * QC, A.psi + (base + (long long)i * A.stride_i) * PC, (unsigned)QC * 8u, bar);
+    }
+}
+
+// tile offset of (i = 0, t, p) for the q-th column
+template <typename G, bool STACKED>
+__device__ __forceinline__ int col_offset(int q, int P) {
+    if (STACKED) { const int t = q / P; return t * G::ST + (q - t * P); }
+    return q;
+}
+
+// ---- phase 1: first factor forward.  Generic: HBM -> registers -> DFT -> shared.  TMA: in place in shared ------------------
+template <int N1, int N2, int QC, int PC, bool STACKED, bool TMA>
 __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long long base, int valid, int tid, int nt) {
+    using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
-    const unsigned stepB = (unsigned)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+    const int SI = G::SI ? G::SI : Q;
+    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
 #pragma unroll 1
     for (int task = tid; task < Q * N2; task += nt) {
         const int b = task / Q, q = task - b * Q;
-        const int t = q / P, p = q - t * P;
+        float2* col = tile + b * SI + col_offset<G, STACKED>(q, P);
         float2 v[N1];
-        if (t < valid) {
-            const float2* src = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+        if (TMA) {
 #pragma unroll
-            for (int a = 0; a < N1; ++a) v[a] = *byte_off(src, stepB, a);
+            for (int a = 0; a < N1; ++a) v[a] = col[a * N2 * SI];
         } else {
+            const int t = q / P, p = q - t * P;
+            if (t < valid) {
+                const float2* src = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
 #pragma unroll
-            for (int a = 0; a < N1; ++a) v[a] = make_float2(0.f, 0.f);
+                for (int a = 0; a < N1; ++a) v[a] = ldg64(src, stepB * a);
+            } else {
+#pragma unroll
+                for (int a = 0; a < N1; ++a) v[a] = make_float2(0.f, 0.f);
+            }
         }
         rtefft::dft_fwd<N1>(v);
-        float2* dst = tile + task;                      // (k1*N2 + b)*Q + q = k1*N2*Q + task
 #pragma unroll
-        for (int k1 = 0; k1 < N1; ++k1) dst[k1 * N2 * Q] = v[k1];
+        for (int k1 = 0; k1 < N1; ++k1) col[k1 * N2 * SI] = v[k1];
     }
 }
 
 // ---- phase 2: twiddle, second factor forward, i k / n, second factor inverse, conjugate twiddle -----------------------
-template <int N1, int N2, int QC, int PC>
+template <int N1, int N2, int QC, int PC, bool STACKED>
 __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, const float2* tw, const float* kap, int tid, int nt) {
+    using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
+    const int SI = G::SI ? G::SI : Q;
 #pragma unroll 1
     for (int task = tid; task < Q * N1; task += nt) {
         const int k1 = task / Q, q = task - k1 * Q;
-        float2* row = tile + (k1 * N2) * Q + q;
+        float2* row = tile + (k1 * N2) * SI + col_offset<G, STACKED>(q, P);
         const float2* twk = tw;
         float2 v[N2];
 #pragma unroll
-        for (int b = 0; b < N2; ++b) v[b] = row[b * Q];
+        for (int b = 0; b < N2; ++b) v[b] = row[b * SI];
 #pragma unroll
         for (int b = 1; b < N2; ++b) { twk += k1; v[b] = rtefft::cmul(v[b], *twk); }
         rtefft::dft_fwd<N2>(v);
         const float* kp = kap + k1;
 #pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) {
-            const float kk = kp[N1 * k2];
-            v[k2] = make_float2(-kk * v[k2].y, kk * v[k2].x);   // * i k
-        }
+        for (int k2 = 0; k2 < N2; ++k2) v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kp[N1 * k2]);   // * i k
         rtefft::dft_inv<N2>(v);
         twk = tw;
 #pragma unroll
         for (int b = 1; b < N2; ++b) { twk += k1; v[b] = rtefft::cmulc(v[b], *twk); }
 #pragma unroll
-        for (int b = 0; b < N2; ++b) row[b * Q] = v[b];
+        for (int b = 0; b < N2; ++b) row[b * SI] = v[b];
     }
 }
 
 // ---- phase 3: first factor inverse: shared now holds D_a psi for every (i, q) -----------------------------------------
-template <int N1, int N2, int QC, int PC>
+template <int N1, int N2, int QC, int PC, bool STACKED>
 __device__ __forceinline__ void phase_inv1(const PassArgs& A, float2* tile, int tid, int nt) {
+    using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
+    const int SI = G::SI ? G::SI : Q;
 #pragma unroll 1
     for (int task = tid; task < Q * N2; task += nt) {
-        float2* col = tile + task;                      // b*Q + q = task
+        const int b = task / Q, q = task - b * Q;
+        float2* col = tile + b * SI + col_offset<G, STACKED>(q, P);
         float2 v[N1];
 #pragma unroll
-        for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * Q];
+        for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
         rtefft::dft_inv<N1>(v);
 #pragma unroll
-        for (int a = 0; a < N1; ++a) col[(a * N2) * Q] = v[a];
+        for (int a = 0; a < N1; ++a) col[(a * N2) * SI] = v[a];
     }
 }
 
@@ -168,13 +258,16 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 }
 
 // ---- phase 4: coupling + accumulate / integrate ---------------------------------------------------------------------
-template <int N1, int N2, int MODE, int E, int QC, int PC>
+template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED>
 __device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile, const float* sig, long long base, int valid,
                                           int tid, int nt, long long pencil0) {
+    using G = Geo<N1, N2, QC, PC, STACKED>;
     constexpr int n = N1 * N2;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
-    const unsigned stepB = (unsigned)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+    const int SI = G::SI ? G::SI : Q;
+    const int ST = G::ST ? G::ST : P;
+    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
 #pragma unroll 1
     for (int task = tid; task < Q * N2; task += nt) {
         const int b = task / Q, q = task - b * Q;
@@ -182,19 +275,20 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile,
         if (t >= valid) continue;
         // this pair's coupling list (unused entries point at the pair itself with zero weights)
         const float2* srow[E];
-        float w00[E], w01[E], w10[E], w11[E];
+        float2 wd[E], ws[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const CplEntry* ce = A.cpl + p * kMaxE + e;
-            srow[e] = tile + b * Q + t * P + __ldg(&ce->src);
-            w00[e] = __ldg(&ce->w00); w01[e] = __ldg(&ce->w01); w10[e] = __ldg(&ce->w10); w11[e] = __ldg(&ce->w11);
+            srow[e] = tile + b * SI + t * ST + __ldg(&ce->src);
+            wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
+            ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
         }
         const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
         const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
         float2* sp = (MODE == MODE_LAST ? A.out : A.acc) + gi;
         float2 r[N1];
 #pragma unroll
-        for (int a = 0; a < N1; ++a) r[a] = *byte_off(lp, stepB, a);
+        for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
         const float* s0 = sig;
         const float* s1 = sig;
         if (MODE == MODE_FIRST) {
@@ -207,17 +301,12 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile,
             float2 T = make_float2(0.f, 0.f);
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                const float2 d = srow[e][(a * N2) * Q];
-                T.x = fmaf(w00[e], d.x, T.x); T.x = fmaf(w01[e], d.y, T.x);
-                T.y = fmaf(w10[e], d.x, T.y); T.y = fmaf(w11[e], d.y, T.y);
+                const float2 d = srow[e][(a * N2) * SI];
+                T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
+                T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
             }
-            if (MODE == MODE_FIRST) {
-                r[a].x = fmaf(r[a].x, s0[a * N2], T.x);
-                r[a].y = fmaf(r[a].y, s1[a * N2], T.y);
-            } else {
-                r[a].x += T.x;
-                r[a].y += T.y;
-            }
+            if (MODE == MODE_FIRST) r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
+            else r[a] = rtefft::cadd(r[a], T);
         }
         if (MODE == MODE_FIRST && A.src_amp != 0.f) {
             // FIRST is the x pass: position along the pencil = x, pencil index = y + ny*z
@@ -237,33 +326,46 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile,
             }
         }
 #pragma unroll
-        for (int a = 0; a < N1; ++a) *byte_off(sp, stepB, a) = r[a];
+        for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
     }
 }
 
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
+    constexpr bool TMA = QC != 0;                               // specialised kernels: tile by TMA bulk copies
+    constexpr bool STACKED = TMA && MODE == MODE_FIRST;         // x pass
+    using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     float2* tile = smem;
-    float2* tw = tile + (size_t)n * Q;
+    float2* tw = tile + (TMA ? (size_t)G::tile_elems : (size_t)n * Q);
     float* kap = reinterpret_cast<float*>(tw + n);
     float* sig = kap + n;
+    __shared__ __align__(8) unsigned long long bar;
     const int tid = threadIdx.x, nt = NTC ? NTC : blockDim.x;
-    for (int i = tid; i < n; i += nt) { tw[i] = A.tw[i]; kap[i] = A.kap[i]; }
     const int group = blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
     const int valid = min(A.TP, A.pencils_per_group - tin * A.TP);
     const long long base = group * A.group_stride + (long long)tin * A.TP * A.stride_t;
-    phase_fwd1<N1, N2, QC, PC>(A, tile, base, valid, tid, nt);
+    if constexpr (TMA) {
+        if (tid == 0) {
+            mbar_init(&bar, 1);
+            mbar_arrive_expect_tx(&bar, (unsigned)n * QC * 8u);
+        }
+        __syncthreads();
+        tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, &bar, tid, nt);
+    }
+    for (int i = tid; i < n; i += nt) { tw[i] = A.tw[i]; kap[i] = A.kap[i]; }
     if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
+    if constexpr (TMA) mbar_wait(&bar, 0);
+    phase_fwd1<N1, N2, QC, PC, STACKED, TMA>(A, tile, base, valid, tid, nt);
     __syncthreads();
-    phase_mid<N1, N2, QC, PC>(A, tile, tw, kap, tid, nt);
+    phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tw, kap, tid, nt);
     __syncthreads();
-    phase_inv1<N1, N2, QC, PC>(A, tile, tid, nt);
+    phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
     __syncthreads();
-    phase_out<N1, N2, MODE, E, QC, PC>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
+    phase_out<N1, N2, MODE, E, QC, PC, STACKED>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
 }
 #endif
 
