@@ -25,8 +25,7 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct AxisTables {
-    float2* tw = nullptr;
-    float* kap = nullptr;
+    float kscale = 0.f;
     CplEntry* cpl = nullptr;
     int n = 0, N1 = 0, N2 = 0, maxcnt = 0;
 };
@@ -362,7 +361,7 @@ constexpr SpecRow kSpec[] = {
 };
 
 size_t pass_smem(int n, int Q, int TP, int nsig, bool first) {
-    size_t b = (size_t)n * Q * sizeof(float2) + (size_t)n * sizeof(float2) + (size_t)n * sizeof(float);
+    size_t b = (size_t)n * Q * sizeof(float2);
     if (first) b += (size_t)nsig * ((size_t)n * TP + 1) * sizeof(float);
     return b;
 }
@@ -466,7 +465,7 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
         A.psi = c->psi; A.acc = c->part; A.out = c->psi;
-        A.tw = c->ax[axis].tw; A.kap = c->ax[axis].kap; A.cpl = c->ax[axis].cpl;
+        A.kscale = c->ax[axis].kscale; A.cpl = c->ax[axis].cpl;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
         A.cdt = c->c * c->dt; A.nsig = c->N + 1;
         A.srcS = c->srcS; A.srcw = c->srcw;
@@ -507,10 +506,34 @@ cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t s) {
     return cudaStreamSynchronize(s);   // v is pageable and about to go out of scope
 }
 
+// Twiddles and wrapped integer wavenumbers of every supported pencil length -> constant memory, once per device.
+cudaError_t upload_constant_tables(int dev) {
+    static bool done[64] = {};
+    if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+    static const int lens[] = {16, 32, 48, 64, 96, 128, 192, 256, 384, 512};
+    std::vector<float2> tw(rtepass::kTableLen);
+    std::vector<float> kw(rtepass::kTableLen);
+    for (int n : lens) {
+        const int off = rtepass::table_offset(n);
+        std::vector<float> t;
+        rtetab::twiddles(n, t);
+        for (int j = 0; j < n; ++j) {
+            tw[off + j] = make_float2(t[2 * j], t[2 * j + 1]);
+            kw[off + j] = (float)((2 * j < n) ? j : ((2 * j == n) ? 0 : j - n));
+        }
+    }
+    cudaError_t e = cudaMemcpyToSymbol(rtepass::c_tw, tw.data(), tw.size() * sizeof(float2));
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyToSymbol(rtepass::c_kw, kw.data(), kw.size() * sizeof(float));
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) done[dev] = true;
+    return cudaSuccess;
+}
+
 void free_ctx(rte_ctx* c) {
     if (!c) return;
     for (int a = 0; a < 3; ++a) {
-        cudaFree(c->ax[a].tw); cudaFree(c->ax[a].kap); cudaFree(c->ax[a].cpl);
+        cudaFree(c->ax[a].cpl);
     }
     cudaFree(c->deg); cudaFree(c->ext_of_slot); cudaFree(c->srcw); cudaFree(c->srcS); cudaFree(c->phi_prev);
     cudaFree(c->red);
@@ -658,18 +681,13 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
     } while (0)
 
     // tables
+    CREATE_TRY(upload_constant_tables(dev));
     const int ext_n[3] = {grid->nx, grid->ny, grid->nz};
     for (int a = 0; a < grid->dim; ++a) {
         AxisTables& T = ctx->ax[a];
         T.n = ext_n[a];
         rtetab::split_of(T.n, T.N1, T.N2);
-        std::vector<float> tw, kap;
-        rtetab::twiddles(T.n, tw);
-        rtetab::kappa_over_n(T.n, dx, kap);
-        std::vector<float2> tw2(T.n);
-        for (int j = 0; j < T.n; ++j) tw2[j] = make_float2(tw[2 * j], tw[2 * j + 1]);
-        CREATE_TRY(upload(&T.tw, tw2, ctx->stream));
-        CREATE_TRY(upload(&T.kap, kap, ctx->stream));
+        T.kscale = (float)(6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n);
         std::vector<std::vector<rtetab::PairEntry>> pe;
         rtetab::pair_coupling(grid->dim, N, a, pe);
         // weights pre-multiplied by -c dt (eq.(11)); unused entries point at the pair itself with zero weights

@@ -44,9 +44,8 @@ struct PassArgs {
     const float2* psi;      // [G][P]  state at t_n (input of the transform)
     float2* acc;            // [G][P]  running accumulator of the new state
     float2* out;            // LAST: where the new state goes (== psi)
-    // tables
-    const float2* tw;       // [n] forward twiddles exp(-2 pi i j/n)
-    const float* kap;       // [n] k_a[j]/n, Nyquist zeroed
+    // tables (twiddles and wrapped integer wavenumbers live in constant memory, see c_tw / c_kw)
+    float kscale;           // 2 pi / (n dx) / n: k_a[j]/n = kscale * wrapped(j)
     const CplEntry* cpl;    // [P][kMaxE], unused entries: src = own pair, weights 0
     // diagonal + source (FIRST)
     const float* sa;        // [G] mu_a in Omega, mu_b in the PML
@@ -68,7 +67,24 @@ struct PassArgs {
     int nx, ny;
 };
 
+// Supported pencil lengths and where their tables start in the constant arrays.
+constexpr int kTableLen = 1728;   // 16+32+48+64+96+128+192+256+384+512
 #ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int table_offset(int n) {
+    return n == 16 ? 0 : n == 32 ? 16 : n == 48 ? 48 : n == 64 ? 96 : n == 96 ? 160 : n == 128 ? 256 : n == 192 ? 384
+         : n == 256 ? 576 : n == 384 ? 832 : n == 512 ? 1216 : -1;
+}
+
+#ifdef __CUDACC__
+
+// c_tw[table_offset(n) + j] = exp(-2 pi i j / n)  (forward twiddles, eq.(8))
+// c_kw[table_offset(n) + j] = j for j < n/2, 0 at j = n/2 (Nyquist, R5), j - n above  (exact in fp32)
+// Read with warp-uniform (or nearly uniform) indices through the constant cache, which keeps these table reads off
+// the shared-memory pipe that bounds the pass kernels.  Filled once per device by rte_create.
+__constant__ float2 c_tw[kTableLen];
+__constant__ float c_kw[kTableLen];
 
 // ---- global memory access with explicit state space (keeps LDG/STG instead of generic LD/ST after byte offsets) ------
 __device__ __forceinline__ float2 ldg64(const float2* p, unsigned long long byte_offset) {
@@ -136,9 +152,13 @@ __device__ __forceinline__ void tile_tma_load(const PassArgs& A, float2* tile, l
             tma_load_1d(dst, src, piece, bar);
         }
     } else {
-        // n rows of Q*8 contiguous bytes (neighbouring pencils of a y/z tile are neighbouring cells)
-        for (int i = tid; i < G::n; i += nt)
-            tma_load_1d(tile + i * QC, A.psi + (base + (long long)i * A.stride_i) * PC, (unsigned)QC * 8u, bar);
+        // n rows of Q*8 contiguous bytes (neighbouring pencils of a y/z tile are neighbouring cells), issued b-major
+        // (i = a*N2 + b); the rows of residue b complete on bar[b], so that the phase-1 columns of residue b can start
+        // while the rest of the tile is still in flight
+        for (int j = tid; j < G::n; j += nt) {
+            const int b = j / N1, a = j - b * N1, i = a * N2 + b;
+            tma_load_1d(tile + i * QC, A.psi + (base + (long long)i * A.stride_i) * PC, (unsigned)QC * 8u, bar + b);
+        }
     }
 }
 
@@ -151,7 +171,8 @@ __device__ __forceinline__ int col_offset(int q, int P) {
 
 // ---- phase 1: first factor forward.  Generic: HBM -> registers -> DFT -> shared.  TMA: in place in shared ------------------
 template <int N1, int N2, int QC, int PC, bool STACKED, bool TMA>
-__device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long long base, int valid, int tid, int nt) {
+__device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long long base, int valid, int tid, int nt,
+                                           unsigned long long* bar) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
@@ -163,6 +184,7 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long
         float2* col = tile + b * SI + col_offset<G, STACKED>(q, P);
         float2 v[N1];
         if (TMA) {
+            mbar_wait(bar + (STACKED ? 0 : b), 0);
 #pragma unroll
             for (int a = 0; a < N1; ++a) v[a] = col[a * N2 * SI];
         } else {
@@ -184,29 +206,29 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long
 
 // ---- phase 2: twiddle, second factor forward, i k / n, second factor inverse, conjugate twiddle -----------------------
 template <int N1, int N2, int QC, int PC, bool STACKED>
-__device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, const float2* tw, const float* kap, int tid, int nt) {
+__device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int tid, int nt) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
+    constexpr int off = table_offset(N1 * N2);
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     const int SI = G::SI ? G::SI : Q;
+    const float kscale = A.kscale;
 #pragma unroll 1
     for (int task = tid; task < Q * N1; task += nt) {
         const int k1 = task / Q, q = task - k1 * Q;
         float2* row = tile + (k1 * N2) * SI + col_offset<G, STACKED>(q, P);
-        const float2* twk = tw;
-        float2 v[N2];
+        float2 v[N2], w[N2];
 #pragma unroll
         for (int b = 0; b < N2; ++b) v[b] = row[b * SI];
 #pragma unroll
-        for (int b = 1; b < N2; ++b) { twk += k1; v[b] = rtefft::cmul(v[b], *twk); }
+        for (int b = 1; b < N2; ++b) { w[b] = c_tw[off + k1 * b]; v[b] = rtefft::cmul(v[b], w[b]); }
         rtefft::dft_fwd<N2>(v);
-        const float* kp = kap + k1;
 #pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kp[N1 * k2]);   // * i k
+        for (int k2 = 0; k2 < N2; ++k2)
+            v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kscale * c_kw[off + k1 + N1 * k2]);   // * i k / n
         rtefft::dft_inv<N2>(v);
-        twk = tw;
 #pragma unroll
-        for (int b = 1; b < N2; ++b) { twk += k1; v[b] = rtefft::cmulc(v[b], *twk); }
+        for (int b = 1; b < N2; ++b) v[b] = rtefft::cmulc(v[b], w[b]);
 #pragma unroll
         for (int b = 0; b < N2; ++b) row[b * SI] = v[b];
     }
@@ -258,8 +280,11 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 }
 
 // ---- phase 4: coupling + accumulate / integrate ---------------------------------------------------------------------
-template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED>
-__device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile, const float* sig, long long base, int valid,
+// FUSED (specialised kernels whose warps own whole rows of the tile, 32 % Q == 0): phase 3 runs here, per warp — the
+// columns (b, all q) a warp transforms are exactly the rows its coupling reads, so a __syncwarp replaces the CTA barrier,
+// the warps drift apart, and the accumulator loads are issued before the inverse DFT and fly under it.
+template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool FUSED>
+__device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
                                           int tid, int nt, long long pencil0) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     constexpr int n = N1 * N2;
@@ -289,6 +314,16 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, const float2* tile,
         float2 r[N1];
 #pragma unroll
         for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+        if (FUSED) {
+            float2* col = tile + b * SI + t * ST + p;
+            float2 v[N1];
+#pragma unroll
+            for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
+            rtefft::dft_inv<N1>(v);
+#pragma unroll
+            for (int a = 0; a < N1; ++a) col[(a * N2) * SI] = v[a];
+            __syncwarp();
+        }
         const float* s0 = sig;
         const float* s1 = sig;
         if (MODE == MODE_FIRST) {
@@ -340,32 +375,32 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     float2* tile = smem;
-    float2* tw = tile + (TMA ? (size_t)G::tile_elems : (size_t)n * Q);
-    float* kap = reinterpret_cast<float*>(tw + n);
-    float* sig = kap + n;
-    __shared__ __align__(8) unsigned long long bar;
+    float* sig = reinterpret_cast<float*>(tile + (TMA ? (size_t)G::tile_elems : (size_t)n * Q));
+    __shared__ __align__(8) unsigned long long bar[N2];
+    constexpr int NBAR = STACKED ? 1 : N2;
+    constexpr bool FUSED = TMA && (32 % (QC ? QC : 7) == 0) && (NTC % 32 == 0);   // a warp owns whole rows in the tail
     const int tid = threadIdx.x, nt = NTC ? NTC : blockDim.x;
     const int group = blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
     const int valid = min(A.TP, A.pencils_per_group - tin * A.TP);
     const long long base = group * A.group_stride + (long long)tin * A.TP * A.stride_t;
     if constexpr (TMA) {
-        if (tid == 0) {
-            mbar_init(&bar, 1);
-            mbar_arrive_expect_tx(&bar, (unsigned)n * QC * 8u);
+        if (tid < NBAR) {
+            mbar_init(&bar[tid], 1);
+            mbar_arrive_expect_tx(&bar[tid], (unsigned)(n / NBAR) * QC * 8u);
         }
         __syncthreads();
-        tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, &bar, tid, nt);
+        tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
-    for (int i = tid; i < n; i += nt) { tw[i] = A.tw[i]; kap[i] = A.kap[i]; }
     if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
-    if constexpr (TMA) mbar_wait(&bar, 0);
-    phase_fwd1<N1, N2, QC, PC, STACKED, TMA>(A, tile, base, valid, tid, nt);
+    phase_fwd1<N1, N2, QC, PC, STACKED, TMA>(A, tile, base, valid, tid, nt, bar);
     __syncthreads();
-    phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tw, kap, tid, nt);
+    phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
     __syncthreads();
-    phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
-    __syncthreads();
-    phase_out<N1, N2, MODE, E, QC, PC, STACKED>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
+    if constexpr (!FUSED) {
+        phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
+        __syncthreads();
+    }
+    phase_out<N1, N2, MODE, E, QC, PC, STACKED, FUSED>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
 }
 #endif
 
