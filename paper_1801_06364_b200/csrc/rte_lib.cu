@@ -703,7 +703,7 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
             if (cnt > T.maxcnt) T.maxcnt = cnt;
             for (int e = 0; e < rtepass::kMaxE; ++e)
                 flat[(size_t)p * rtepass::kMaxE + e] =
-                    e < cnt ? CplEntry{(float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w11),
+                    (e < cnt && pe[p][e].src >= 0) ? CplEntry{(float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w11),
                                        (float)(mcdt * pe[p][e].w01), (float)(mcdt * pe[p][e].w10), pe[p][e].src, 0}
                             : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
         }

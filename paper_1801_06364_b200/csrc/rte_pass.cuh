@@ -170,25 +170,56 @@ __device__ __forceinline__ int col_offset(int q, int P) {
 }
 
 // ---- phase 1: first factor forward.  Generic: HBM -> registers -> DFT -> shared.  TMA: in place in shared ------------------
-template <int N1, int N2, int QC, int PC, bool STACKED, bool TMA>
+// CF ("couple first", specialised kernels): the streaming coupling is applied HERE, to the transform's input —
+//   -c dt T_c = D_a ( sum_c' w^a_{cc'} psi_c' )      (constant weights commute with D_a; R18)
+// so a column gathers its <= E source pairs from the freshly loaded tile, and the tail needs no neighbour data at all:
+// one shared-memory store and E loads per element become E loads, and the tail runs without any barrier.  The
+// gather reads rows that other columns of the same rows overwrite, hence the fence between gather and store: the rows
+// of one residue b are owned by one warp (32 % Q == 0) or by one round of the whole CTA (nt % Q == 0).
+template <int N1, int N2, int E, int QC, int PC, bool STACKED, bool TMA, bool CF>
 __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long long base, int valid, int tid, int nt,
                                            unsigned long long* bar) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     const int SI = G::SI ? G::SI : Q;
+    const int ST = G::ST ? G::ST : P;
     const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
 #pragma unroll 1
     for (int task = tid; task < Q * N2; task += nt) {
         const int b = task / Q, q = task - b * Q;
-        float2* col = tile + b * SI + col_offset<G, STACKED>(q, P);
+        const int t = q / P, p = q - t * P;
+        float2* col = tile + b * SI + t * ST + p;
         float2 v[N1];
-        if (TMA) {
+        if (CF) {
+            const float2* srow[E];
+            float2 wd[E], ws[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const CplEntry* ce = A.cpl + p * kMaxE + e;
+                srow[e] = tile + b * SI + t * ST + __ldg(&ce->src);
+                wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
+                ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
+            }
+            mbar_wait(bar + (STACKED ? 0 : b), 0);
+#pragma unroll
+            for (int a = 0; a < N1; ++a) {
+                float2 u = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const float2 d = srow[e][(a * N2) * SI];
+                    u = rtefft::cfma_diag(wd[e].x, wd[e].y, d, u);
+                    u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
+                }
+                v[a] = u;
+            }
+            if (QC && 32 % (QC ? QC : 1) == 0) __syncwarp();
+            else __syncthreads();
+        } else if (TMA) {
             mbar_wait(bar + (STACKED ? 0 : b), 0);
 #pragma unroll
             for (int a = 0; a < N1; ++a) v[a] = col[a * N2 * SI];
         } else {
-            const int t = q / P, p = q - t * P;
             if (t < valid) {
                 const float2* src = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
 #pragma unroll
@@ -283,7 +314,8 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // FUSED (specialised kernels whose warps own whole rows of the tile, 32 % Q == 0): phase 3 runs here, per warp — the
 // columns (b, all q) a warp transforms are exactly the rows its coupling reads, so a __syncwarp replaces the CTA barrier,
 // the warps drift apart, and the accumulator loads are issued before the inverse DFT and fly under it.
-template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool FUSED>
+// CF: the coupling was applied in phase 1; the tail is  acc (+)= IDFT_{N1}(column)  straight from registers.
+template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool FUSED, bool CF>
 __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
                                           int tid, int nt, long long pencil0) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
@@ -301,12 +333,14 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
         // this pair's coupling list (unused entries point at the pair itself with zero weights)
         const float2* srow[E];
         float2 wd[E], ws[E];
+        if (!CF) {
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const CplEntry* ce = A.cpl + p * kMaxE + e;
-            srow[e] = tile + b * SI + t * ST + __ldg(&ce->src);
-            wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
-            ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
+            for (int e = 0; e < E; ++e) {
+                const CplEntry* ce = A.cpl + p * kMaxE + e;
+                srow[e] = tile + b * SI + t * ST + __ldg(&ce->src);
+                wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
+                ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
+            }
         }
         const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
         const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
@@ -314,15 +348,17 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
         float2 r[N1];
 #pragma unroll
         for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
-        if (FUSED) {
+        float2 v[N1];
+        if (FUSED || CF) {
             float2* col = tile + b * SI + t * ST + p;
-            float2 v[N1];
 #pragma unroll
             for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
             rtefft::dft_inv<N1>(v);
+            if (!CF) {
 #pragma unroll
-            for (int a = 0; a < N1; ++a) col[(a * N2) * SI] = v[a];
-            __syncwarp();
+                for (int a = 0; a < N1; ++a) col[(a * N2) * SI] = v[a];
+                __syncwarp();
+            }
         }
         const float* s0 = sig;
         const float* s1 = sig;
@@ -334,11 +370,14 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
 #pragma unroll
         for (int a = 0; a < N1; ++a) {
             float2 T = make_float2(0.f, 0.f);
+            if (CF) T = v[a];
+            else {
 #pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const float2 d = srow[e][(a * N2) * SI];
-                T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
-                T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
+                for (int e = 0; e < E; ++e) {
+                    const float2 d = srow[e][(a * N2) * SI];
+                    T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
+                    T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
+                }
             }
             if (MODE == MODE_FIRST) r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
             else r[a] = rtefft::cadd(r[a], T);
@@ -378,7 +417,9 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
     float* sig = reinterpret_cast<float*>(tile + (TMA ? (size_t)G::tile_elems : (size_t)n * Q));
     __shared__ __align__(8) unsigned long long bar[N2];
     constexpr int NBAR = STACKED ? 1 : N2;
-    constexpr bool FUSED = TMA && (32 % (QC ? QC : 7) == 0) && (NTC % 32 == 0);   // a warp owns whole rows in the tail
+    constexpr bool FUSED = TMA && (32 % (QC ? QC : 7) == 0) && (NTC % 32 == 0);   // a warp owns whole rows of the tile
+    // couple first: rows of one residue are owned by a warp, or by one full round of the CTA's task loop
+    constexpr bool CF = FUSED || (TMA && NTC % (QC ? QC : 7) == 0 && (QC * N2) % (NTC ? NTC : 1) == 0);
     const int tid = threadIdx.x, nt = NTC ? NTC : blockDim.x;
     const int group = blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
     const int valid = min(A.TP, A.pencils_per_group - tin * A.TP);
@@ -392,15 +433,15 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
     if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
-    phase_fwd1<N1, N2, QC, PC, STACKED, TMA>(A, tile, base, valid, tid, nt, bar);
+    phase_fwd1<N1, N2, E, QC, PC, STACKED, TMA, CF>(A, tile, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
     __syncthreads();
-    if constexpr (!FUSED) {
+    if constexpr (!FUSED && !CF) {
         phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
         __syncthreads();
     }
-    phase_out<N1, N2, MODE, E, QC, PC, STACKED, FUSED>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
+    phase_out<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
 }
 #endif
 

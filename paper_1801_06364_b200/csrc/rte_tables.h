@@ -16,6 +16,9 @@
 #pragma once
 #include <cmath>
 #include <cstdint>
+#include <map>
+#include <mutex>
+#include <utility>
 #include <vector>
 
 namespace rtetab {
@@ -114,8 +117,9 @@ inline void coupling_real(int dim, int N, std::vector<double> A[3]) {
     }
 }
 
-// internal slot order: ext_of_slot[s] = external coefficient index (or -1 for the pad), deg_of_slot[s] = l (2-D: m)
-inline void slot_order(int dim, int N, std::vector<int>& ext_of_slot, std::vector<int>& deg_of_slot) {
+// base slot order (before the bank-conflict permutation of pair positions, see PairLayout below):
+// ext_of_slot[s] = external coefficient index (or -1 for the pad), deg_of_slot[s] = l (2-D: m)
+inline void base_slot_order(int dim, int N, std::vector<int>& ext_of_slot, std::vector<int>& deg_of_slot) {
     ext_of_slot.clear(); deg_of_slot.clear();
     if (dim == 3) {
         for (int l = 0; l <= N; ++l) { ext_of_slot.push_back(ia3(l, 0)); deg_of_slot.push_back(l); }
@@ -138,12 +142,11 @@ inline void slot_order(int dim, int N, std::vector<int>& ext_of_slot, std::vecto
 struct PairEntry { int src; float w00, w01, w10, w11; };   // out.x += w00 in.x + w01 in.y ; out.y += w10 in.x + w11 in.y
 
 // coupling regrouped by pairs: for output pair po the list of (source pair, 2x2 block)
-inline void pair_coupling(int dim, int N, int axis, std::vector<std::vector<PairEntry>>& out) {
+inline void pair_coupling_of(int dim, int N, int axis, const std::vector<int>& ext,
+                             std::vector<std::vector<PairEntry>>& out) {
     std::vector<double> A[3];
     coupling_real(dim, N, A);
     const int C = num_coeffs(dim, N);
-    std::vector<int> ext, deg;
-    slot_order(dim, N, ext, deg);
     const int P = (int)ext.size() / 2;
     out.assign(P, {});
     for (int po = 0; po < P; ++po)
@@ -158,6 +161,167 @@ inline void pair_coupling(int dim, int N, int axis, std::vector<std::vector<Pair
                     if (w[r][c] != 0.0) any = true;
                 }
             if (any) out[po].push_back({ps, (float)w[0][0], (float)w[0][1], (float)w[1][0], (float)w[1][1]});
+        }
+}
+
+// ---- pair layout: positions of the pairs inside a cell record, and the entry order of the coupling lists ----------------
+// The specialised pass kernels gather, per coupling entry e, one 8-byte element per lane from the shared-memory tile:
+// lane (row i, pencil t, position pp) reads tile[i*Q + t*P + pos(src_e(pair at pp))] (x pass with several pencils per
+// tile: pencils stacked with pitch = P mod 16 (mod 16)).  A 64-bit shared load is served half-warp by half-warp; two
+// lanes of a half-warp that hit the same 8-byte bank (address mod 16) at different addresses cost an extra wavefront.
+// Both the position of every pair in the record and the order of a pair's entries are free, so they are chosen here to
+// minimise those extra wavefronts (deterministic simulated annealing; the pair that holds coefficient 0 stays at
+// position 0 because the fluence read-out takes slot 0).  Pure layout: no arithmetic of the method depends on it.
+struct PairLayout {
+    int P = 0;
+    std::vector<int> pos;                          // pos[base pair] = position in the record
+    std::vector<int> inv;                          // inv[position] = base pair
+    std::vector<std::vector<int>> slots[3];        // slots[axis][position][e] = source POSITION, or -1 (unused)
+    int cost0 = 0, cost = 0, ideal = 0;            // modelled wavefronts: base layout, chosen layout, conflict-free
+};
+
+inline int layout_tp(int dim, int N) {   // pencils per tile assumed by the model (the specialised kernels' choice)
+    const int P = (dim == 3 ? ((N + 1) + ((N + 1) % 2)) / 2 + N * (N + 1) / 2 : N + 1);
+    int tp = 1;
+    while (tp * P < 32 && tp < 8) tp *= 2;
+    return tp;
+}
+
+inline int layout_cost(int P, int TP, int naxes, const int* E, const std::vector<int>& pos, const std::vector<int>& inv,
+                       const std::vector<std::vector<int>>* src /* [axis][base pair][e] base pair or -1 */) {
+    const int Q = TP * P;
+    int g = 32, h = Q;
+    while (h) { const int r = g % h; g = h; h = r; }
+    const int period = 32 * Q / g;                 // tasks after which the warp/row alignment repeats
+    int tot = 0;
+    for (int axis = 0; axis < naxes; ++axis)
+        for (int e = 0; e < E[axis]; ++e)
+            for (int w0 = 0; w0 < period; w0 += 16) {          // one half-warp at a time
+                int worst = 1;
+                std::vector<int> seen[16];
+                for (int lane = 0; lane < 16; ++lane) {
+                    const int task = w0 + lane, b = task / Q, q = task - b * Q, t = q / P, pp = q - t * P;
+                    const int pr = inv[pp];
+                    int s = src[axis][pr][e];
+                    if (s < 0) s = pr;
+                    const int addr = (axis == 0 && TP > 1) ? t * (P % 16) + b * P + pos[s] + 4096 * t : b * Q + t * P + pos[s];
+                    const int bank = addr & 15;
+                    bool dup = false;
+                    for (int a : seen[bank]) if (a == addr) dup = true;
+                    if (!dup) { seen[bank].push_back(addr); if ((int)seen[bank].size() > worst) worst = (int)seen[bank].size(); }
+                }
+                tot += worst;
+            }
+    return tot;
+}
+
+inline const PairLayout& pair_layout(int dim, int N) {
+    static std::mutex mu;
+    static std::map<std::pair<int, int>, PairLayout> cache;
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = cache.find({dim, N});
+    if (it != cache.end()) return it->second;
+    PairLayout L;
+    std::vector<int> ext, deg;
+    base_slot_order(dim, N, ext, deg);
+    const int P = (int)ext.size() / 2, naxes = dim, TP = layout_tp(dim, N);
+    L.P = P;
+    // coupling structure in base pair indices, padded with -1 to E entries per axis
+    int E[3] = {4, 4, 4};
+    std::vector<std::vector<int>> src[3];
+    for (int a = 0; a < naxes; ++a) {
+        std::vector<std::vector<PairEntry>> pe;
+        pair_coupling_of(dim, N, a, ext, pe);
+        size_t mx = 0;
+        for (auto& v : pe) mx = v.size() > mx ? v.size() : mx;
+        if (dim == 3 && a == 2 && mx <= 3) E[a] = 3;            // the z kernels read 3 entries (rte_lib.cu launch_spec)
+        if ((int)mx > E[a]) E[a] = (int)mx;
+        src[a].assign(P, {});
+        for (int p = 0; p < P; ++p) {
+            for (auto& en : pe[p]) src[a][p].push_back(en.src);
+            while ((int)src[a][p].size() < E[a]) src[a][p].push_back(-1);
+        }
+    }
+    std::vector<int> pos(P), inv(P);
+    for (int p = 0; p < P; ++p) pos[p] = inv[p] = p;
+    L.cost0 = layout_cost(P, TP, naxes, E, pos, inv, src);
+    {
+        int g = 32, h = TP * P;
+        while (h) { const int r = g % h; g = h; h = r; }
+        int ne = 0;
+        for (int a = 0; a < naxes; ++a) ne += E[a];
+        L.ideal = ne * (32 * TP * P / g) / 16;
+    }
+    // deterministic annealing: swap two pair positions (never position 0) or permute one pair's entry order
+    uint64_t rng = 0x9E3779B97F4A7C15ull ^ ((uint64_t)dim << 32) ^ (uint64_t)N;
+    auto next = [&]() { rng = rng * 6364136223846793005ull + 1442695040888963407ull; return (uint32_t)(rng >> 33); };
+    int cur = L.cost0, best = cur;
+    std::vector<int> best_pos = pos;
+    std::vector<std::vector<int>> best_src[3] = {src[0], src[1], src[2]};
+    double T = 2.0;
+    const int iters = (P > 2 && cur > L.ideal) ? 20000 : 0;
+    for (int itn = 0; itn < iters && best > L.ideal; ++itn) {
+        const bool swap_move = (next() & 1) && P > 2;
+        int i = 0, j = 0, a = 0, p = 0;
+        std::vector<int> old;
+        if (swap_move) {
+            i = 1 + (int)(next() % (uint32_t)(P - 1));
+            j = 1 + (int)(next() % (uint32_t)(P - 1));
+            if (i == j) continue;
+            std::swap(pos[i], pos[j]);
+            inv[pos[i]] = i; inv[pos[j]] = j;
+        } else {
+            a = (int)(next() % (uint32_t)naxes); p = (int)(next() % (uint32_t)P);
+            old = src[a][p];
+            for (int k = E[a] - 1; k > 0; --k) std::swap(src[a][p][k], src[a][p][next() % (uint32_t)(k + 1)]);
+        }
+        const int c = layout_cost(P, TP, naxes, E, pos, inv, src);
+        const double u = (double)(next() & 0xFFFFFF) / 16777216.0;
+        if (c <= cur || u < std::exp((double)(cur - c) / T)) cur = c;
+        else if (swap_move) { std::swap(pos[i], pos[j]); inv[pos[i]] = i; inv[pos[j]] = j; }
+        else src[a][p] = old;
+        T = T * 0.9995 > 0.05 ? T * 0.9995 : 0.05;
+        if (cur < best) { best = cur; best_pos = pos; for (int k = 0; k < 3; ++k) best_src[k] = src[k]; }
+    }
+    L.cost = best;
+    L.pos = best_pos;
+    L.inv.assign(P, 0);
+    for (int p = 0; p < P; ++p) L.inv[L.pos[p]] = p;
+    for (int a = 0; a < naxes; ++a) {
+        L.slots[a].assign(P, {});
+        for (int pp = 0; pp < P; ++pp)
+            for (int s : best_src[a][L.inv[pp]]) L.slots[a][pp].push_back(s < 0 ? -1 : L.pos[s]);
+    }
+    return cache.emplace(std::make_pair(dim, N), std::move(L)).first->second;
+}
+
+// internal slot order = base order with the pairs moved to their layout positions
+inline void slot_order(int dim, int N, std::vector<int>& ext_of_slot, std::vector<int>& deg_of_slot) {
+    std::vector<int> ext, deg;
+    base_slot_order(dim, N, ext, deg);
+    const PairLayout& L = pair_layout(dim, N);
+    ext_of_slot.assign(ext.size(), -1); deg_of_slot.assign(deg.size(), 0);
+    for (int p = 0; p < L.P; ++p)
+        for (int h = 0; h < 2; ++h) {
+            ext_of_slot[2 * L.pos[p] + h] = ext[2 * p + h];
+            deg_of_slot[2 * L.pos[p] + h] = deg[2 * p + h];
+        }
+}
+
+// coupling by pair POSITION, entries in the layout's order (gaps, src = -1, carry zero weights)
+inline void pair_coupling(int dim, int N, int axis, std::vector<std::vector<PairEntry>>& out) {
+    std::vector<int> ext, deg;
+    slot_order(dim, N, ext, deg);
+    std::vector<std::vector<PairEntry>> pe;
+    pair_coupling_of(dim, N, axis, ext, pe);
+    const PairLayout& L = pair_layout(dim, N);
+    out.assign(L.P, {});
+    for (int pp = 0; pp < L.P; ++pp)
+        for (int s : L.slots[axis][pp]) {
+            PairEntry en{-1, 0.f, 0.f, 0.f, 0.f};
+            if (s >= 0)
+                for (auto& c : pe[pp]) if (c.src == s) en = c;
+            out[pp].push_back(en);
         }
 }
 
