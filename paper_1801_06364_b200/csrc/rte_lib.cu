@@ -82,7 +82,7 @@ bool extent_ok(int n) { int a, b; return rtetab::split_of(n, a, b); }
 
 int padded_coeffs(int dim, int N) {
     std::vector<int> e, d;
-    rtetab::slot_order(dim, N, e, d);
+    rtetab::base_slot_order(dim, N, e, d);
     return (int)e.size();
 }
 
@@ -383,7 +383,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     A.P = P;
     for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
         if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
-            !(axis == c->grid.dim - 1 && c->grid.dim == 3 && T.maxcnt > 3)) {
+            !(axis == c->grid.dim - 1 && c->grid.dim == 3 && T.maxcnt > 2)) {
             L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
             break;
         }
@@ -441,7 +441,7 @@ cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaSt
     }
 }
 
-// E = 3 on the z axis of 3-D runs (fan-in of the z coupling is at most 3 pairs), 4 otherwise
+// E = 2 on the z axis of 3-D runs (fan-in of the z coupling is at most 2 pairs, rte_tables.h), 4 otherwise
 template <int MODE, int E>
 cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     switch (spec) {
@@ -482,7 +482,7 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
                             : launch_generic<rtepass::MODE_FIRST>(n, A, L, c->stream);
         } else if (axis == naxes - 1) {
             if (L.spec >= 0)
-                e = naxes == 3 ? launch_spec<rtepass::MODE_LAST, 3>(L.spec, A, L, c->stream)
+                e = naxes == 3 ? launch_spec<rtepass::MODE_LAST, 2>(L.spec, A, L, c->stream)
                                : launch_spec<rtepass::MODE_LAST, 4>(L.spec, A, L, c->stream);
             else e = launch_generic<rtepass::MODE_LAST>(n, A, L, c->stream);
         } else {

@@ -8,8 +8,8 @@
 //
 // Internal storage: the C real fields are regrouped into P = Cp/2 "pairs" so that one complex FFT differentiates two
 // real fields at once (D_a is a real operator, so D(u + i v) = Du + i Dv):
-//   3-D: the m = 0 fields a_l^0 (l = 0..N) come first, two per pair (a zero pad field completes the last pair when
-//        N+1 is odd); then one pair (a_l^m, b_l^m) for every m >= 1, l >= m.  This makes every pair with m >= 1 the
+//   3-D: the m = 0 fields a_l^0 (l = 0..N) come first, two per pair, even with even and odd with odd degree (a zero
+//        pad field completes the last pair when N+1 is odd); then one pair (a_l^m, b_l^m) for every m >= 1, l >= m.  This makes every pair with m >= 1 the
 //        paper's complex coefficient psi_l^m up to a factor, so x/y/z coupling maps pairs to pairs.
 //   2-D: (a_0, pad), then (a_m, b_m), m = 1..N.
 // Slot 0 is always coefficient 0 (the fluence).
@@ -122,8 +122,21 @@ inline void coupling_real(int dim, int N, std::vector<double> A[3]) {
 inline void base_slot_order(int dim, int N, std::vector<int>& ext_of_slot, std::vector<int>& deg_of_slot) {
     ext_of_slot.clear(); deg_of_slot.clear();
     if (dim == 3) {
-        for (int l = 0; l <= N; ++l) { ext_of_slot.push_back(ia3(l, 0)); deg_of_slot.push_back(l); }
-        if ((N + 1) % 2) { ext_of_slot.push_back(-1); deg_of_slot.push_back(0); }
+        // m = 0 fields: even degrees paired among themselves, odd degrees among themselves (a_0,a_2), (a_4,a_6), ...,
+        // (a_1,a_3), ...; a left-over even and a left-over odd degree share a pair, a single left-over gets the pad.
+        // The z coupling links l to l+-1, i.e. even to odd, so a pair then has at most 2 source pairs on the z axis
+        // (3 with (a_l, a_l+1) pairs, which couple to themselves) and the z kernels gather 2 entries instead of 3.
+        std::vector<int> ev, od, rest;
+        for (int l = 0; l <= N; ++l) (l % 2 ? od : ev).push_back(l);
+        auto emit = [&](std::vector<int>& v) {
+            size_t k = 0;
+            for (; k + 1 < v.size(); k += 2)
+                for (int h = 0; h < 2; ++h) { ext_of_slot.push_back(ia3(v[k + h], 0)); deg_of_slot.push_back(v[k + h]); }
+            if (k < v.size()) rest.push_back(v[k]);
+        };
+        emit(ev); emit(od);
+        for (int l : rest) { ext_of_slot.push_back(ia3(l, 0)); deg_of_slot.push_back(l); }
+        if (rest.size() % 2) { ext_of_slot.push_back(-1); deg_of_slot.push_back(0); }
         for (int m = 1; m <= N; ++m)
             for (int l = m; l <= N; ++l) {
                 ext_of_slot.push_back(ia3(l, m)); deg_of_slot.push_back(l);
@@ -234,7 +247,7 @@ inline const PairLayout& pair_layout(int dim, int N) {
         pair_coupling_of(dim, N, a, ext, pe);
         size_t mx = 0;
         for (auto& v : pe) mx = v.size() > mx ? v.size() : mx;
-        if (dim == 3 && a == 2 && mx <= 3) E[a] = 3;            // the z kernels read 3 entries (rte_lib.cu launch_spec)
+        if (dim == 3 && a == 2 && mx <= 2) E[a] = 2;            // the z kernels read 2 entries (rte_lib.cu launch_spec)
         if ((int)mx > E[a]) E[a] = (int)mx;
         src[a].assign(P, {});
         for (int p = 0; p < P; ++p) {
@@ -259,7 +272,7 @@ inline const PairLayout& pair_layout(int dim, int N) {
     std::vector<int> best_pos = pos;
     std::vector<std::vector<int>> best_src[3] = {src[0], src[1], src[2]};
     double T = 2.0;
-    const int iters = (P > 2 && cur > L.ideal) ? 20000 : 0;
+    const int iters = (P > 2 && P <= 40 && cur > L.ideal) ? 20000 : 0;   // larger records: base layout (generic kernels)
     for (int itn = 0; itn < iters && best > L.ideal; ++itn) {
         const bool swap_move = (next() & 1) && P > 2;
         int i = 0, j = 0, a = 0, p = 0;
