@@ -316,8 +316,8 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // the warps drift apart, and the accumulator loads are issued before the inverse DFT and fly under it.
 // CF: the coupling was applied in phase 1; the tail is  acc (+)= IDFT_{N1}(column)  straight from registers.
 template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool FUSED, bool CF>
-__device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
-                                          int tid, int nt, long long pencil0) {
+__device__ __forceinline__ void tail_task(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
+                                          int task, long long pencil0, float2 (&r)[N1], bool loaded) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     constexpr int n = N1 * N2;
     const int P = PC ? PC : A.P;
@@ -325,11 +325,10 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
     const int SI = G::SI ? G::SI : Q;
     const int ST = G::ST ? G::ST : P;
     const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
-#pragma unroll 1
-    for (int task = tid; task < Q * N2; task += nt) {
+    {
         const int b = task / Q, q = task - b * Q;
         const int t = q / P, p = q - t * P;
-        if (t >= valid) continue;
+        if (t >= valid) return;
         // this pair's coupling list (unused entries point at the pair itself with zero weights)
         const float2* srow[E];
         float2 wd[E], ws[E];
@@ -345,9 +344,10 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
         const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
         const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
         float2* sp = (MODE == MODE_LAST ? A.out : A.acc) + gi;
-        float2 r[N1];
+        if (!loaded) {
 #pragma unroll
-        for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+            for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+        }
         float2 v[N1];
         if (FUSED || CF) {
             float2* col = tile + b * SI + t * ST + p;
@@ -404,6 +404,20 @@ __device__ __forceinline__ void phase_out(const PassArgs& A, float2* tile, const
     }
 }
 
+// the global loads of one tail task (accumulator rows; psi itself in the FIRST pass): issued as early as possible
+template <int N1, int N2, int MODE, int QC, int PC>
+__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]) {
+    const int P = PC ? PC : A.P;
+    const int Q = QC ? QC : A.TP * P;
+    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+    const int b = task / Q, q = task - b * Q;
+    const int t = q / P, p = q - t * P;
+    const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
+#pragma unroll
+    for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+}
+
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
     extern __shared__ __align__(128) float2 smem[];
@@ -436,12 +450,31 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
     phase_fwd1<N1, N2, E, QC, PC, STACKED, TMA, CF>(A, tile, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
-    __syncthreads();
-    if constexpr (!FUSED && !CF) {
-        phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
+    const long long pencil0 = (long long)blockIdx.x * A.TP;
+    if constexpr (CF) {
+        // the first tail task's global loads are issued BEFORE the barrier, so they fly while the slower warps finish
+        // phase 2 (the loads depend on nothing in shared memory; valid == TP in the specialised kernels)
+        float2 r[N1];
+        tail_load<N1, N2, MODE, QC, PC>(A, base, tid, r);
         __syncthreads();
+        tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, tid, pencil0, r, true);
+#pragma unroll 1
+        for (int task = tid + nt; task < Q * N2; task += nt) {
+            float2 r2[N1];
+            tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, task, pencil0, r2, false);
+        }
+    } else {
+        __syncthreads();
+        if constexpr (!FUSED) {
+            phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
+            __syncthreads();
+        }
+#pragma unroll 1
+        for (int task = tid; task < Q * N2; task += nt) {
+            float2 r[N1];
+            tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, task, pencil0, r, false);
+        }
     }
-    phase_out<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, tid, nt, (long long)blockIdx.x * A.TP);
 }
 #endif
 
