@@ -73,11 +73,11 @@ def hbm_peak():
 # algorithmic bytes: S = 4*C*G bytes is one fp32 state
 # ---------------------------------------------------------------------------------------------------------------------
 def algorithmic_bytes(cfg):
-    """Bytes each per-axis kernel must move per launch, and per step.  x pass: read psi, write partial (2 S);
-    middle pass (3-D y): read psi + partial, write partial (3 S); last pass: read psi + partial, write psi (3 S)
-    plus the three per-cell coefficient maps (12 B/cell).  2-D has no middle pass."""
+    """Bytes each per-axis kernel must move per launch, and per step.  x pass: read psi and the three per-cell
+    coefficient maps (12 B/cell), write the Euler accumulator (2 S + 12 G); middle pass (3-D y): read psi +
+    accumulator, write accumulator (3 S); last pass: read psi + accumulator, write psi (3 S).  2-D has no middle pass."""
     S = 4 * cfg.C * cfg.G
-    per_axis = [2 * S, 3 * S, 3 * S + 12 * cfg.G] if cfg.dim == 3 else [2 * S, 3 * S + 12 * cfg.G, 0]
+    per_axis = [2 * S + 12 * cfg.G, 3 * S, 3 * S] if cfg.dim == 3 else [2 * S + 12 * cfg.G, 3 * S, 0]
     return per_axis, sum(per_axis)
 
 
@@ -305,9 +305,10 @@ def measure_workload(rte, wl, cfg, torch, dev, steps, warmup, dist=None, sampler
 def roofline_of(cfg, res, peak, peak_kind):
     per_axis, per_step = algorithmic_bytes(cfg)
     naxes = cfg.dim
-    names = ["pass_x (DFT-ik-IDFT + coupling, first)", "pass_y (middle, accumulates)", "pass_z (last: + sigma_l, PML, source, Euler)"]
+    names = ["pass_x (first: coupling, DFT-ik-IDFT, sigma_l, PML, source -> Euler accumulator)",
+             "pass_y (middle: accumulates)", "pass_z (last: writes the new state)"]
     if cfg.dim == 2:
-        names = [names[0], "pass_y (last: + sigma_l, PML, source, Euler)", ""]
+        names = [names[0], "pass_y (last: writes the new state)", ""]
     dom = max(range(naxes), key=lambda a: res["ms_axis"][a])
     ach = per_axis[dom] / (res["ms_axis"][dom] * 1e-3) / 1e9
     kernels = []
