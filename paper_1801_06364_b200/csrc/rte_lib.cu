@@ -25,7 +25,6 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct AxisTables {
-    float kscale = 0.f;
     CplEntry* cpl = nullptr;
     int n = 0, N1 = 0, N2 = 0, maxcnt = 0;
 };
@@ -465,7 +464,7 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
         A.psi = c->psi; A.acc = c->part; A.out = c->psi;
-        A.kscale = c->ax[axis].kscale; A.cpl = c->ax[axis].cpl;
+        A.cpl = c->ax[axis].cpl;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
         A.cdt = c->c * c->dt; A.nsig = c->N + 1;
         A.srcS = c->srcS; A.srcw = c->srcw;
@@ -687,11 +686,11 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
         AxisTables& T = ctx->ax[a];
         T.n = ext_n[a];
         rtetab::split_of(T.n, T.N1, T.N2);
-        T.kscale = (float)(6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n);
         std::vector<std::vector<rtetab::PairEntry>> pe;
         rtetab::pair_coupling(grid->dim, N, a, pe);
         // weights pre-multiplied by -c dt (eq.(11)); unused entries point at the pair itself with zero weights
-        const double mcdt = -(double)c * (double)dt;
+        // -c dt (eq.(11)) times the axis' wavenumber unit and 1/n (the kernel multiplies by the integer wavenumber only)
+        const double mcdt = -(double)c * (double)dt * 6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n;
         std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE);
         T.maxcnt = 0;
         for (int p = 0; p < ctx->P; ++p) {

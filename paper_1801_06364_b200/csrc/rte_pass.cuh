@@ -34,7 +34,7 @@ constexpr int kMaxE = 4;   // max source pairs per output pair and axis (checked
 
 // One 2x2 real block of the coupling: T.x += wd0 d.x + ws0 d.y ; T.y += wd1 d.y + ws1 d.x  (wd = diagonal (w00, w11),
 // ws = off-diagonal (w01, w10); stored as the two register pairs of the packed FFMA2 form).  Weights already
-// multiplied by -c dt.
+// multiplied by -c dt * 2 pi / (n_a dx) / n_a (Euler step, wavenumber unit and inverse-DFT normalisation of the axis).
 struct alignas(8) CplEntry { float wd0, wd1, ws0, ws1; int src; int pad_; };
 
 enum { MODE_FIRST = 0, MODE_MIDDLE = 1, MODE_LAST = 2 };
@@ -45,7 +45,6 @@ struct PassArgs {
     float2* acc;            // [G][P]  running accumulator of the new state
     float2* out;            // LAST: where the new state goes (== psi)
     // tables (twiddles and wrapped integer wavenumbers live in constant memory, see c_tw / c_kw)
-    float kscale;           // 2 pi / (n dx) / n: k_a[j]/n = kscale * wrapped(j)
     const CplEntry* cpl;    // [P][kMaxE], unused entries: src = own pair, weights 0
     // diagonal + source (FIRST)
     const float* sa;        // [G] mu_a in Omega, mu_b in the PML
@@ -243,7 +242,6 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     const int SI = G::SI ? G::SI : Q;
-    const float kscale = A.kscale;
 #pragma unroll 1
     for (int task = tid; task < Q * N1; task += nt) {
         const int k1 = task / Q, q = task - k1 * Q;
@@ -256,7 +254,7 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
         rtefft::dft_fwd<N2>(v);
 #pragma unroll
         for (int k2 = 0; k2 < N2; ++k2)
-            v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kscale * c_kw[off + k1 + N1 * k2]);   // * i k / n
+            v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), c_kw[off + k1 + N1 * k2]);   // * i * wrapped(k); 2 pi/(n dx)/n is in the weights
         rtefft::dft_inv<N2>(v);
 #pragma unroll
         for (int b = 1; b < N2; ++b) v[b] = rtefft::cmulc(v[b], w[b]);
