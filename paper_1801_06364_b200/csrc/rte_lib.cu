@@ -12,6 +12,7 @@
 #include <limits>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "rte_pass.cuh"
@@ -359,9 +360,9 @@ constexpr SpecRow kSpec[] = {
     {64, 4, 8, 256},     // cfg0: 64^2 P_3 (2-D)
 };
 
-size_t pass_smem(int n, int Q, int TP, int nsig, bool first) {
+size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
     size_t b = (size_t)n * Q * sizeof(float2);
-    if (first) b += (size_t)nsig * ((size_t)n * TP + 1) * sizeof(float);
+    if (diag) b += (size_t)nsig * ((size_t)n * TP + 1) * sizeof(float);   // per-tile table of the Euler diagonal
     return b;
 }
 
@@ -376,7 +377,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     } else { A.stride_i = nx * ny; A.stride_t = 1; A.group_stride = 0; A.pencils_per_group = nx * ny; }
     const AxisTables& T = c->ax[axis];
     const int P = c->P, n = T.n;
-    const bool first = axis == 0;
+    const bool first = axis == 0, diag = first;   // the x pass carries the Euler diagonal table
     LaunchPlan L{};
     L.spec = -1;
     A.P = P;
@@ -389,7 +390,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     if (L.spec < 0) {
         int tp = 1;
         while (tp * P < 32 && tp < 8) tp *= 2;
-        while (tp > 1 && pass_smem(n, tp * P, tp, c->N + 1, first) > 100 * 1024) tp /= 2;
+        while (tp > 1 && pass_smem(n, tp * P, tp, c->N + 1, diag) > 100 * 1024) tp /= 2;
         while (tp > 1 && tp > A.pencils_per_group) tp /= 2;
         const int Q = tp * P;
         const int T1 = Q * T.N2, T2 = Q * T.N1;
@@ -405,7 +406,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     A.TP = L.TP;
     A.tiles_per_group = (A.pencils_per_group + L.TP - 1) / L.TP;
     L.blocks = groups * A.tiles_per_group;
-    L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, first);
+    L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, diag);
     if (L.spec >= 0 && first && L.TP > 1) L.smem += (size_t)L.TP * (P % 16) * sizeof(float2);   // stacked-layout padding
     return L;
 }
@@ -463,7 +464,7 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
     const int naxes = c->grid.dim;
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
-        A.psi = c->psi; A.acc = c->part; A.out = c->psi;
+        A.psi = c->psi; A.acc = c->part;
         A.cpl = c->ax[axis].cpl;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
         A.cdt = c->c * c->dt; A.nsig = c->N + 1;
@@ -479,19 +480,20 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
                 A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, (double)c->steps * (double)c->dt));
             e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream)
                             : launch_generic<rtepass::MODE_FIRST>(n, A, L, c->stream);
-        } else if (axis == naxes - 1) {
-            if (L.spec >= 0)
-                e = naxes == 3 ? launch_spec<rtepass::MODE_LAST, 2>(L.spec, A, L, c->stream)
-                               : launch_spec<rtepass::MODE_LAST, 4>(L.spec, A, L, c->stream);
-            else e = launch_generic<rtepass::MODE_LAST>(n, A, L, c->stream);
+        } else if (axis == 2) {
+            // z axis: coupling fan-in 2 (rte_tables.h); plan_pass falls back to the generic kernel otherwise
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 2>(L.spec, A, L, c->stream)
+                            : launch_generic<rtepass::MODE_ACC>(n, A, L, c->stream);
         } else {
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_MIDDLE, 4>(L.spec, A, L, c->stream)
-                            : launch_generic<rtepass::MODE_MIDDLE>(n, A, L, c->stream);
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 4>(L.spec, A, L, c->stream)
+                            : launch_generic<rtepass::MODE_ACC>(n, A, L, c->stream);
         }
         if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
         c->launches += 1;
         if (ev) cudaEventRecord(ev[axis], c->stream);
     }
+    // the accumulator now holds psi^{n+1}: the two state buffers trade places
+    std::swap(c->psi, c->part);
     c->steps += 1;
     return RTE_OK;
 }

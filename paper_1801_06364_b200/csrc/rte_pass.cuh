@@ -1,18 +1,23 @@
 // rte_pass.cuh — the per-axis pencil kernel of the P_N pseudospectral RTE step (sm_100a).
 //
-// One launch handles one axis a of the step (PAPER.md:123-127 re-designed):
-//   1. load a tile of TP adjacent pencils (all coefficients of every cell on the pencil) straight from HBM into
-//      registers (N1 loads in flight per thread) and do the first factor of DFT_n      eq.(7)-(8)
-//   2. second factor (N2-point), multiply by i k_a / n (Nyquist zeroed), inverse second factor  eq.(10)
-//   3. inverse first factor -> D_a psi on the pencil, kept in shared memory
-//   4. streaming coupling  -c dt T_c = sum_c' w^a_{cc'} D_a psi_c'  (sparse l+-1, m, m+-1; the weights arrive
-//      pre-multiplied by -c dt)                                                        eq.(6)/(10)
-//      and, depending on MODE, the running forward-Euler accumulator `acc` (eq.(11)):
-//        FIRST   acc  = psi (1 - c dt sigma_l) - c dt T_x + c dt q   (x pass: scattering diagonal eq.(9), PML
-//                                                                    eq.(12), source)
-//        MIDDLE  acc += -c dt T_y                                    (y pass in 3-D)
-//        LAST    psi  = acc - c dt T_a                               (last axis; in place: tiles are disjoint and
-//                                                                    every read of a tile precedes its writes)
+// One launch handles one axis a of the step (PAPER.md:123-127 re-designed).  The state is double
+// buffered: every pass READS psi^n and ACCUMULATES into the buffer that becomes psi^{n+1} (eq.(11)):
+//        FIRST (x axis)  new  = psi (1 - c dt sigma_l) + c dt q - c dt T_x   (scattering diagonal eq.(9), PML eq.(12),
+//                                                                            source; plain stores)
+//        ACC (other axes) new += -c dt T_a
+// with  -c dt T_c = D_a ( sum_c' w^a_{cc'} psi_c' )  the streaming coupling (sparse l+-1, m, m+-1; eq.(6)/(10),
+// PAPER.md:73-78) and D_a = IDFT (i k_a) DFT the spectral derivative along the axis (eq.(7)-(8),(10)).
+// Specialised kernels (the BASELINE configurations; compile-time geometry):
+//   0. the psi tile (TP adjacent pencils, all pairs of every cell) arrives in shared memory by TMA bulk copies
+//   1. gather + couple the <= E source pairs of every column, first factor of DFT_n (N1-point), in place
+//   2. twiddle, second factor (N2-point), multiply by i k_a (Nyquist zeroed), inverse second factor, conjugate twiddle
+//   3. inverse first factor in registers, then
+//      ACC:   ONE fire-and-forget vector reduction per element into the new buffer (red.global.add.v2.f32, SASS
+//             REDG.ADD.F32x2, performed by the L2 at full HBM rate): the SM never waits for the accumulator, and since
+//             every address receives exactly one reduction per pass the result does not depend on scheduling;
+//      FIRST: psi is read again (L2 hit), combined with the Euler diagonal and the source, and stored.
+// Generic kernels (any supported extent / order): registers -> DFT -> shared, phases 2, 3, coupling from the
+// differentiated pencil, accumulator by load / add / store.
 // The coefficient fields are stored cell-major, [cell][P] float2 ("pairs", see rte_tables.h), so a pencil along any
 // axis is a sequence of P*8-byte contiguous chunks and one complex FFT differentiates two real fields.
 //
@@ -37,13 +42,12 @@ constexpr int kMaxE = 4;   // max source pairs per output pair and axis (checked
 // multiplied by -c dt * 2 pi / (n_a dx) / n_a (Euler step, wavenumber unit and inverse-DFT normalisation of the axis).
 struct alignas(8) CplEntry { float wd0, wd1, ws0, ws1; int src; int pad_; };
 
-enum { MODE_FIRST = 0, MODE_MIDDLE = 1, MODE_LAST = 2 };
+enum { MODE_ACC = 0, MODE_FIRST = 1 };
 
 struct PassArgs {
     // fields
     const float2* psi;      // [G][P]  state at t_n (input of the transform)
-    float2* acc;            // [G][P]  running accumulator of the new state
-    float2* out;            // LAST: where the new state goes (== psi)
+    float2* acc;            // [G][P]  accumulator: becomes the state at t_{n+1} after the last pass
     // tables (twiddles and wrapped integer wavenumbers live in constant memory, see c_tw / c_kw)
     const CplEntry* cpl;    // [P][kMaxE], unused entries: src = own pair, weights 0
     // diagonal + source (FIRST)
@@ -93,6 +97,12 @@ __device__ __forceinline__ float2 ldg64(const float2* p, unsigned long long byte
 }
 __device__ __forceinline__ void stg64(float2* p, unsigned long long byte_offset, float2 v) {
     asm volatile("st.global.v2.f32 [%0], {%1,%2};" ::"l"(reinterpret_cast<char*>(p) + byte_offset), "f"(v.x), "f"(v.y) : "memory");
+}
+
+// fire-and-forget  *p += v  on both halves (performed at the L2; flushes subnormals to zero, which is far below the
+// parity tolerance).  One reduction per address per pass: deterministic.
+__device__ __forceinline__ void red_add64(float2* p, unsigned long long byte_offset, float2 v) {
+    asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(reinterpret_cast<char*>(p) + byte_offset), "f"(v.x), "f"(v.y) : "memory");
 }
 
 // ---- mbarrier + TMA bulk copy (global -> shared) ----------------------------------------------------------------------
@@ -168,6 +178,32 @@ __device__ __forceinline__ int col_offset(int q, int P) {
     return q;
 }
 
+// ---- source term along one x pencil (FIRST is the x pass): c dt f(t_n) w_c S(r) for the cells inside the source box ------
+struct SourceRow {
+    bool on = false;
+    float sw0 = 0.f, sw1 = 0.f;
+    const float* S = nullptr;      // S at x = box origin of this pencil's row of the box
+    int x0 = 0, ext = 0;
+    // pencil = y + ny*z of the pencil, p = pair
+    __device__ __forceinline__ SourceRow(const PassArgs& A, long long pencil, int p) {
+        if (A.src_amp == 0.f) return;
+        const int by = (int)(pencil % A.ny) - A.src_org[1], bz = (int)(pencil / A.ny) - A.src_org[2];
+        if (by < 0 || by >= A.src_ext[1] || bz < 0 || bz >= A.src_ext[2]) return;
+        on = true;
+        sw0 = __ldg(A.srcw + 2 * p) * A.src_amp; sw1 = __ldg(A.srcw + 2 * p + 1) * A.src_amp;
+        S = A.srcS + ((size_t)bz * A.src_ext[1] + by) * A.src_ext[0];
+        x0 = A.src_org[0]; ext = A.src_ext[0];
+    }
+    __device__ __forceinline__ void add(int x, float2& e) const {
+        if (!on) return;
+        const int bx = x - x0;
+        if (bx >= 0 && bx < ext) {
+            const float v = __ldg(S + bx);
+            e.x = fmaf(sw0, v, e.x); e.y = fmaf(sw1, v, e.y);
+        }
+    }
+};
+
 // ---- phase 1: first factor forward.  Generic: HBM -> registers -> DFT -> shared.  TMA: in place in shared ------------------
 // CF ("couple first", specialised kernels): the streaming coupling is applied HERE, to the transform's input —
 //   -c dt T_c = D_a ( sum_c' w^a_{cc'} psi_c' )      (constant weights commute with D_a; R18)
@@ -175,9 +211,9 @@ __device__ __forceinline__ int col_offset(int q, int P) {
 // one shared-memory store and E loads per element become E loads, and the tail runs without any barrier.  The
 // gather reads rows that other columns of the same rows overwrite, hence the fence between gather and store: the rows
 // of one residue b are owned by one warp (32 % Q == 0) or by one round of the whole CTA (nt % Q == 0).
-template <int N1, int N2, int E, int QC, int PC, bool STACKED, bool TMA, bool CF>
-__device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long long base, int valid, int tid, int nt,
-                                           unsigned long long* bar) {
+template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool TMA, bool CF>
+__device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
+                                           int tid, int nt, unsigned long long* bar) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
@@ -214,10 +250,6 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, long
             }
             if (QC && 32 % (QC ? QC : 1) == 0) __syncwarp();
             else __syncthreads();
-        } else if (TMA) {
-            mbar_wait(bar + (STACKED ? 0 : b), 0);
-#pragma unroll
-            for (int a = 0; a < N1; ++a) v[a] = col[a * N2 * SI];
         } else {
             if (t < valid) {
                 const float2* src = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
@@ -308,134 +340,132 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
     }
 }
 
-// ---- phase 4: coupling + accumulate / integrate ---------------------------------------------------------------------
-// FUSED (specialised kernels whose warps own whole rows of the tile, 32 % Q == 0): phase 3 runs here, per warp — the
-// columns (b, all q) a warp transforms are exactly the rows its coupling reads, so a __syncwarp replaces the CTA barrier,
-// the warps drift apart, and the accumulator loads are issued before the inverse DFT and fly under it.
-// CF: the coupling was applied in phase 1; the tail is  acc (+)= IDFT_{N1}(column)  straight from registers.
-template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool FUSED, bool CF>
-__device__ __forceinline__ void tail_task(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
-                                          int task, long long pencil0, float2 (&r)[N1], bool loaded) {
+// ---- tail, specialised kernels: inverse first factor in registers, then one store / vector reduction per element ---------
+// (the coupling was applied in phase 1; every thread owns its column, so there is no barrier and no neighbour data)
+// FIRST: r holds the column's own psi (loaded by tail_load, the first task's before the phase-2 barrier).
+template <int N1, int N2, int MODE, int QC, int PC, bool STACKED>
+__device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile, const float* sig, long long base, int task,
+                                          long long pencil0, float2 (&r)[N1]) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     constexpr int n = N1 * N2;
-    const int P = PC ? PC : A.P;
-    const int Q = QC ? QC : A.TP * P;
-    const int SI = G::SI ? G::SI : Q;
-    const int ST = G::ST ? G::ST : P;
-    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
-    {
-        const int b = task / Q, q = task - b * Q;
-        const int t = q / P, p = q - t * P;
-        if (t >= valid) return;
-        // this pair's coupling list (unused entries point at the pair itself with zero weights)
-        const float2* srow[E];
-        float2 wd[E], ws[E];
-        if (!CF) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const CplEntry* ce = A.cpl + p * kMaxE + e;
-                srow[e] = tile + b * SI + t * ST + __ldg(&ce->src);
-                wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
-                ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
-            }
-        }
-        const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
-        const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
-        float2* sp = (MODE == MODE_LAST ? A.out : A.acc) + gi;
-        if (!loaded) {
-#pragma unroll
-            for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
-        }
-        float2 v[N1];
-        if (FUSED || CF) {
-            float2* col = tile + b * SI + t * ST + p;
-#pragma unroll
-            for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
-            rtefft::dft_inv<N1>(v);
-            if (!CF) {
-#pragma unroll
-                for (int a = 0; a < N1; ++a) col[(a * N2) * SI] = v[a];
-                __syncwarp();
-            }
-        }
-        const float* s0 = sig;
-        const float* s1 = sig;
-        if (MODE == MODE_FIRST) {
-            const int ncell1 = n * A.TP + 1;
-            s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
-            s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
-        }
-#pragma unroll
-        for (int a = 0; a < N1; ++a) {
-            float2 T = make_float2(0.f, 0.f);
-            if (CF) T = v[a];
-            else {
-#pragma unroll
-                for (int e = 0; e < E; ++e) {
-                    const float2 d = srow[e][(a * N2) * SI];
-                    T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
-                    T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
-                }
-            }
-            if (MODE == MODE_FIRST) r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
-            else r[a] = rtefft::cadd(r[a], T);
-        }
-        if (MODE == MODE_FIRST && A.src_amp != 0.f) {
-            // FIRST is the x pass: position along the pencil = x, pencil index = y + ny*z
-            const long long pen = pencil0 + t;
-            const int by = (int)(pen % A.ny) - A.src_org[1], bz = (int)(pen / A.ny) - A.src_org[2];
-            if (by >= 0 && by < A.src_ext[1] && bz >= 0 && bz < A.src_ext[2]) {
-                const float sw0 = __ldg(A.srcw + 2 * p) * A.src_amp, sw1 = __ldg(A.srcw + 2 * p + 1) * A.src_amp;
-                const float* Srow = A.srcS + ((size_t)bz * A.src_ext[1] + by) * A.src_ext[0];
-#pragma unroll
-                for (int a = 0; a < N1; ++a) {
-                    const int bx = a * N2 + b - A.src_org[0];
-                    if (bx >= 0 && bx < A.src_ext[0]) {
-                        const float S = __ldg(Srow + bx);
-                        r[a].x = fmaf(sw0, S, r[a].x); r[a].y = fmaf(sw1, S, r[a].y);
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
-    }
-}
-
-// the global loads of one tail task (accumulator rows; psi itself in the FIRST pass): issued as early as possible
-template <int N1, int N2, int MODE, int QC, int PC>
-__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]) {
-    const int P = PC ? PC : A.P;
-    const int Q = QC ? QC : A.TP * P;
+    constexpr int P = PC, Q = QC, SI = G::SI, ST = G::ST;
     const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
     const int b = task / Q, q = task - b * Q;
     const int t = q / P, p = q - t * P;
-    const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
-    const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
+    const float2* col = tile + b * SI + t * ST + p;
+    float2 v[N1];
+#pragma unroll
+    for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
+    rtefft::dft_inv<N1>(v);
+    float2* sp = A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    if (MODE == MODE_FIRST) {
+        const int ncell1 = n * A.TP + 1;
+        const float* s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
+        const float* s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
+        const SourceRow src(A, pencil0 + t, p);
+#pragma unroll
+        for (int a = 0; a < N1; ++a) {
+            float2 e = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], v[a]);
+            src.add(a * N2 + b, e);
+            stg64(sp, stepB * a, e);
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < N1; ++a) red_add64(sp, stepB * a, v[a]);
+    }
+}
+
+// the psi re-read of one FIRST tail task, issued as early as possible
+template <int N1, int N2, int QC, int PC>
+__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]) {
+    constexpr int P = PC, Q = QC;
+    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+    const int b = task / Q, q = task - b * Q;
+    const int t = q / P, p = q - t * P;
+    const float2* lp = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
 #pragma unroll
     for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+}
+
+// ---- tail, generic kernels: coupling from the differentiated pencil + accumulate / integrate -----------------------------
+template <int N1, int N2, int MODE, int E>
+__device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* tile, const float* sig, long long base, int valid,
+                                             int task, long long pencil0) {
+    constexpr int n = N1 * N2;
+    const int P = A.P;
+    const int Q = A.TP * P;
+    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+    const int b = task / Q, q = task - b * Q;
+    const int t = q / P, p = q - t * P;
+    if (t >= valid) return;
+    // this pair's coupling list (unused entries point at the pair itself with zero weights)
+    const float2* srow[E];
+    float2 wd[E], ws[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const CplEntry* ce = A.cpl + p * kMaxE + e;
+        srow[e] = tile + b * Q + t * P + __ldg(&ce->src);
+        wd[e] = __ldg(reinterpret_cast<const float2*>(&ce->wd0));
+        ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
+    }
+    const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
+    float2* sp = A.acc + gi;
+    float2 r[N1];
+#pragma unroll
+    for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+    const float* s0 = sig;
+    const float* s1 = sig;
+    if (MODE == MODE_FIRST) {
+        const int ncell1 = n * A.TP + 1;
+        s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
+        s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
+    }
+    const SourceRow src(A, pencil0 + t, p);
+#pragma unroll
+    for (int a = 0; a < N1; ++a) {
+        float2 T = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const float2 d = srow[e][(a * N2) * Q];
+            T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
+            T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
+        }
+        if (MODE == MODE_FIRST) {
+            r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
+            src.add(a * N2 + b, r[a]);
+        } else {
+            r[a] = rtefft::cadd(r[a], T);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
 }
 
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
-    constexpr bool TMA = QC != 0;                               // specialised kernels: tile by TMA bulk copies
-    constexpr bool STACKED = TMA && MODE == MODE_FIRST;         // x pass
+    constexpr bool TMA = QC != 0;                                             // specialised kernels: tile by TMA bulk copies
+    constexpr bool STACKED = TMA && MODE == MODE_FIRST && (QC / (PC ? PC : 1)) > 1;   // x pass (FIRST) with several pencils
     using G = Geo<N1, N2, QC, PC, STACKED>;
+    // couple first needs the rows of one residue owned by a warp (32 % Q == 0) or by one full round of the CTA's task
+    // loop (nt % Q == 0, whole rounds); all specialised configurations qualify (checked here at compile time)
+    constexpr bool CF = TMA;
+    static_assert(!TMA || ((32 % (QC ? QC : 1) == 0 && NTC % 32 == 0) ||
+                           (NTC % (QC ? QC : 1) == 0 && (QC * N2) % (NTC ? NTC : 1) == 0)),
+                  "specialised geometry must let a warp or a CTA round own whole tile rows");
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     float2* tile = smem;
     float* sig = reinterpret_cast<float*>(tile + (TMA ? (size_t)G::tile_elems : (size_t)n * Q));
     __shared__ __align__(8) unsigned long long bar[N2];
     constexpr int NBAR = STACKED ? 1 : N2;
-    constexpr bool FUSED = TMA && (32 % (QC ? QC : 7) == 0) && (NTC % 32 == 0);   // a warp owns whole rows of the tile
-    // couple first: rows of one residue are owned by a warp, or by one full round of the CTA's task loop
-    constexpr bool CF = FUSED || (TMA && NTC % (QC ? QC : 7) == 0 && (QC * N2) % (NTC ? NTC : 1) == 0);
     const int tid = threadIdx.x, nt = NTC ? NTC : blockDim.x;
     const int group = blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
     const int valid = min(A.TP, A.pencils_per_group - tin * A.TP);
     const long long base = group * A.group_stride + (long long)tin * A.TP * A.stride_t;
+    const long long pencil0 = (long long)blockIdx.x * A.TP;
     if constexpr (TMA) {
         if (tid < NBAR) {
             mbar_init(&bar[tid], 1);
@@ -444,34 +474,29 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         __syncthreads();
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
-    if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
-    phase_fwd1<N1, N2, E, QC, PC, STACKED, TMA, CF>(A, tile, base, valid, tid, nt, bar);
+    if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
+    phase_fwd1<N1, N2, MODE, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
-    const long long pencil0 = (long long)blockIdx.x * A.TP;
     if constexpr (CF) {
-        // the first tail task's global loads are issued BEFORE the barrier, so they fly while the slower warps finish
-        // phase 2 (the loads depend on nothing in shared memory; valid == TP in the specialised kernels)
         float2 r[N1];
-        tail_load<N1, N2, MODE, QC, PC>(A, base, tid, r);
+        // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
+        // phase 2 (the loads depend on nothing in shared memory)
+        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
         __syncthreads();
-        tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, tid, pencil0, r, true);
+        tail_spec<N1, N2, MODE, QC, PC, STACKED>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, task, pencil0, r2, false);
+            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
+            tail_spec<N1, N2, MODE, QC, PC, STACKED>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();
-        if constexpr (!FUSED) {
-            phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
-            __syncthreads();
-        }
+        phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
+        __syncthreads();
 #pragma unroll 1
-        for (int task = tid; task < Q * N2; task += nt) {
-            float2 r[N1];
-            tail_task<N1, N2, MODE, E, QC, PC, STACKED, FUSED, CF>(A, tile, sig, base, valid, task, pencil0, r, false);
-        }
+        for (int task = tid; task < Q * N2; task += nt) tail_generic<N1, N2, MODE, E>(A, tile, sig, base, valid, task, pencil0);
     }
 }
 #endif
