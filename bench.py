@@ -74,8 +74,8 @@ def hbm_peak():
 # ---------------------------------------------------------------------------------------------------------------------
 def algorithmic_bytes(cfg):
     """Bytes each per-axis kernel must move per launch, and per step.  x pass: read psi and the three per-cell
-    coefficient maps (12 B/cell), write the Euler accumulator (2 S + 12 G); middle pass (3-D y): read psi +
-    accumulator, write accumulator (3 S); last pass: read psi + accumulator, write psi (3 S).  2-D has no middle pass."""
+    coefficient maps (12 B/cell), write the new buffer (2 S + 12 G); every other pass: read psi, read + write the new
+    buffer (the reductions are read-modify-write in the L2: 3 S).  2-D has no z pass."""
     S = 4 * cfg.C * cfg.G
     per_axis = [2 * S + 12 * cfg.G, 3 * S, 3 * S] if cfg.dim == 3 else [2 * S + 12 * cfg.G, 3 * S, 0]
     return per_axis, sum(per_axis)
@@ -305,10 +305,9 @@ def measure_workload(rte, wl, cfg, torch, dev, steps, warmup, dist=None, sampler
 def roofline_of(cfg, res, peak, peak_kind):
     per_axis, per_step = algorithmic_bytes(cfg)
     naxes = cfg.dim
-    names = ["pass_x (first: coupling, DFT-ik-IDFT, sigma_l, PML, source -> Euler accumulator)",
-             "pass_y (middle: accumulates)", "pass_z (last: writes the new state)"]
-    if cfg.dim == 2:
-        names = [names[0], "pass_y (last: writes the new state)", ""]
+    names = ["pass_x (first: coupling, DFT-ik-IDFT, sigma_l, PML, source -> stores the new buffer)",
+             "pass_y (coupling, DFT-ik-IDFT -> vector reductions into the new buffer)",
+             "pass_z (coupling, DFT-ik-IDFT -> vector reductions into the new buffer)"]
     dom = max(range(naxes), key=lambda a: res["ms_axis"][a])
     ach = per_axis[dom] / (res["ms_axis"][dom] * 1e-3) / 1e9
     kernels = []
@@ -327,7 +326,7 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {}
+TRAFFIC_NCU = {"cfg4": {0: 29698156000, 1: 43432037000, 2: 43430344000}}   # profiles/r1e_cfg4_pass_kernels.md
 
 
 def run_ours(args, wl, cfg):

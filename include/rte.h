@@ -75,6 +75,15 @@ int rte_num_coeffs(int dim, int N);
  * A_out[c*C + c'] (host, C*C doubles) with T_c = sum_c' A[c][c'] d psi_c' / d x_axis; axis 0=x, 1=y, 2=z. */
 int rte_coupling_table(int dim, int N, int axis, double* A_out_host);
 
+/* Internal storage layout (host only; no device call).  The C fields are stored cell-major in Cp = 2*P slots, two
+ * real fields per "pair" (one complex FFT differentiates both).  The position of each pair
+ * in a cell record and the order of its coupling entries are chosen to make the kernels' shared-memory gathers
+ * bank-conflict free.  Outputs (any may be NULL): Cp_out = number of slots; ext_of_slot_host[Cp] = external
+ * coefficient index stored in each slot, -1 for a zero pad slot (slot 0 is always coefficient 0, the fluence);
+ * cost_host[3] = modelled gather wavefronts {natural order, chosen layout, conflict-free ideal}.
+ * Returns RTE_EINVAL for dim not in {2,3} or N < 1. */
+int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* cost_host);
+
 /* Bytes of device workspace rte_create needs for this grid and order (state, partial sums, coefficient maps). */
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out);
 

@@ -44,6 +44,7 @@ _vp, _i, _f = C.c_void_p, C.c_int, C.c_float
 _i3 = C.POINTER(C.c_int)
 _lib.rte_num_coeffs.argtypes = [_i, _i]
 _lib.rte_coupling_table.argtypes = [_i, _i, _i, C.POINTER(C.c_double)]
+_lib.rte_storage_layout.argtypes = [_i, _i, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]
 _lib.rte_workspace_bytes.argtypes = [C.POINTER(rte_grid), _i, C.POINTER(C.c_size_t)]
 _lib.rte_create.argtypes = [C.POINTER(_vp), C.POINTER(rte_grid), _i, _f, _f, _f, C.POINTER(rte_media),
                             C.POINTER(rte_pml), _vp, C.c_size_t, _vp]
@@ -68,7 +69,7 @@ _lib.rte_media_ellipsoids.argtypes = [C.POINTER(rte_grid), _f, C.POINTER(C.c_flo
 _lib.rte_media_lognormal.argtypes = [C.POINTER(rte_grid), _f, C.c_uint64, _f, _f, _f, _vp, _vp, _vp]
 _lib.rte_pml_profile.argtypes = [C.POINTER(rte_grid), C.POINTER(rte_pml), _vp, _vp, _vp]
 
-EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_workspace_bytes", "rte_create", "rte_destroy",
+EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_workspace_bytes", "rte_create", "rte_destroy",
             "rte_set_state", "rte_get_state", "rte_set_state_host", "rte_get_state_host", "rte_reset_time",
             "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_profile", "rte_fluence", "rte_fluence_host",
             "rte_fluence_change", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
@@ -112,6 +113,17 @@ def rte_coupling_table(dim, N, axis):
     A = np.zeros((n, n))
     _check(_lib.rte_coupling_table(dim, N, axis, A.ctypes.data_as(C.POINTER(C.c_double))))
     return A
+
+
+def rte_storage_layout(dim, N):
+    """(ext_of_slot[Cp] int array, (cost_natural, cost_chosen, cost_ideal)) — host only, see include/rte.h."""
+    import numpy as np
+    cp = _i(0)
+    _check(_lib.rte_storage_layout(dim, N, C.byref(cp), None, None))
+    ext = np.zeros(cp.value, dtype=np.int32)
+    cost = (_i * 3)()
+    _check(_lib.rte_storage_layout(dim, N, C.byref(cp), ext.ctypes.data_as(C.POINTER(_i)), cost))
+    return ext, tuple(cost)
 
 
 def rte_workspace_bytes(grid, N):

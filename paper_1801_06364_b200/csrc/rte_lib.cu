@@ -602,6 +602,19 @@ int rte_coupling_table(int dim, int N, int axis, double* A_out_host) {
     return RTE_OK;
 }
 
+int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* cost_host) {
+    if (rtetab::num_coeffs(dim, N) < 0) return RTE_EINVAL;
+    std::vector<int> eos, deg;
+    rtetab::slot_order(dim, N, eos, deg);
+    if (Cp_out) *Cp_out = (int)eos.size();
+    if (ext_of_slot_host) std::memcpy(ext_of_slot_host, eos.data(), eos.size() * sizeof(int));
+    if (cost_host) {
+        const rtetab::PairLayout& L = rtetab::pair_layout(dim, N);
+        cost_host[0] = L.cost0; cost_host[1] = L.cost; cost_host[2] = L.ideal;
+    }
+    return RTE_OK;
+}
+
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out) {
     if (!bytes_out || check_grid(grid) != RTE_OK || N < 1) return RTE_EINVAL;
     const size_t G = (size_t)grid->nx * grid->ny * grid->nz;

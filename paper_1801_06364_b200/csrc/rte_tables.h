@@ -200,31 +200,35 @@ inline int layout_tp(int dim, int N) {   // pencils per tile assumed by the mode
     return tp;
 }
 
-inline int layout_cost(int P, int TP, int naxes, const int* E, const std::vector<int>& pos, const std::vector<int>& inv,
-                       const std::vector<std::vector<int>>* src /* [axis][base pair][e] base pair or -1 */) {
+// modelled wavefronts of ONE axis' gathers for a candidate layout
+inline int layout_cost_axis(int P, int TP, int axis, int E, const std::vector<int>& pos, const std::vector<int>& inv,
+                            const std::vector<std::vector<int>>& src /* [base pair][e] base pair or -1 */) {
     const int Q = TP * P;
     int g = 32, h = Q;
     while (h) { const int r = g % h; g = h; h = r; }
     const int period = 32 * Q / g;                 // tasks after which the warp/row alignment repeats
+    const bool stacked = axis == 0 && TP > 1;
     int tot = 0;
-    for (int axis = 0; axis < naxes; ++axis)
-        for (int e = 0; e < E[axis]; ++e)
-            for (int w0 = 0; w0 < period; w0 += 16) {          // one half-warp at a time
-                int worst = 1;
-                std::vector<int> seen[16];
-                for (int lane = 0; lane < 16; ++lane) {
-                    const int task = w0 + lane, b = task / Q, q = task - b * Q, t = q / P, pp = q - t * P;
-                    const int pr = inv[pp];
-                    int s = src[axis][pr][e];
-                    if (s < 0) s = pr;
-                    const int addr = (axis == 0 && TP > 1) ? t * (P % 16) + b * P + pos[s] + 4096 * t : b * Q + t * P + pos[s];
-                    const int bank = addr & 15;
-                    bool dup = false;
-                    for (int a : seen[bank]) if (a == addr) dup = true;
-                    if (!dup) { seen[bank].push_back(addr); if ((int)seen[bank].size() > worst) worst = (int)seen[bank].size(); }
-                }
-                tot += worst;
+    for (int w0 = 0; w0 < period; w0 += 16) {      // one half-warp at a time
+        int abase[16], pr[16];
+        for (int lane = 0; lane < 16; ++lane) {
+            const int task = w0 + lane, b = task / Q, q = task - b * Q, t = q / P;
+            pr[lane] = inv[q - t * P];
+            abase[lane] = stacked ? t * (P % 16) + b * P + 4096 * t : b * Q + t * P;
+        }
+        for (int e = 0; e < E; ++e) {
+            int worst = 1, cnt[16] = {0}, seen[16][16];
+            for (int lane = 0; lane < 16; ++lane) {
+                int s = src[pr[lane]][e];
+                if (s < 0) s = pr[lane];
+                const int addr = abase[lane] + pos[s], bank = addr & 15;
+                bool dup = false;
+                for (int k = 0; k < cnt[bank]; ++k) if (seen[bank][k] == addr) dup = true;
+                if (!dup) { seen[bank][cnt[bank]++] = addr; if (cnt[bank] > worst) worst = cnt[bank]; }
             }
+            tot += worst;
+        }
+    }
     return tot;
 }
 
@@ -257,7 +261,9 @@ inline const PairLayout& pair_layout(int dim, int N) {
     }
     std::vector<int> pos(P), inv(P);
     for (int p = 0; p < P; ++p) pos[p] = inv[p] = p;
-    L.cost0 = layout_cost(P, TP, naxes, E, pos, inv, src);
+    int cax[3] = {0, 0, 0};
+    for (int a = 0; a < naxes; ++a) cax[a] = layout_cost_axis(P, TP, a, E[a], pos, inv, src[a]);
+    L.cost0 = cax[0] + cax[1] + cax[2];
     {
         int g = 32, h = TP * P;
         while (h) { const int r = g % h; g = h; h = r; }
@@ -288,9 +294,12 @@ inline const PairLayout& pair_layout(int dim, int N) {
             old = src[a][p];
             for (int k = E[a] - 1; k > 0; --k) std::swap(src[a][p][k], src[a][p][next() % (uint32_t)(k + 1)]);
         }
-        const int c = layout_cost(P, TP, naxes, E, pos, inv, src);
+        int nax[3] = {cax[0], cax[1], cax[2]};
+        for (int k = 0; k < naxes; ++k)
+            if (swap_move || k == a) nax[k] = layout_cost_axis(P, TP, k, E[k], pos, inv, src[k]);
+        const int c = nax[0] + nax[1] + nax[2];
         const double u = (double)(next() & 0xFFFFFF) / 16777216.0;
-        if (c <= cur || u < std::exp((double)(cur - c) / T)) cur = c;
+        if (c <= cur || u < std::exp((double)(cur - c) / T)) { cur = c; for (int k = 0; k < 3; ++k) cax[k] = nax[k]; }
         else if (swap_move) { std::swap(pos[i], pos[j]); inv[pos[i]] = i; inv[pos[j]] = j; }
         else src[a][p] = old;
         T = T * 0.9995 > 0.05 ? T * 0.9995 : 0.05;

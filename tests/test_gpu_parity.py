@@ -352,6 +352,41 @@ def test_host_buffer_entry_points_and_state_roundtrip():
     assert abs(rte.rte_time_ps(ctx) - 4 * cfg.dt) < 1e-9
 
 
+@pytest.mark.parametrize("grid,N", [((128, 16, 16), 3), ((32, 32, 32), 4)])
+def test_double_buffer_odd_steps_and_determinism(grid, N):
+    """The state is double buffered (each pass reads psi^n and reduces into the buffer that becomes psi^{n+1}; the
+    accumulating passes use fire-and-forget red.global.add — one reduction per address per pass).  (i) Reading the state
+    and the fluence after an ODD number of steps, through device and host entry points, then stepping on, matches the
+    oracle stepped straight through; (ii) two identical runs are bit-identical (no scheduling dependence)."""
+    cfg = wl.Config("dbuf", 3, grid[0], grid[1], grid[2], N, 0.2, 0.002, 0.3, 5, (2, 0.01, 2.0), "homogeneous", "none", 0)
+    rng = np.random.default_rng(11)
+    mu_a = rng.uniform(0.01, 0.5, cfg.shape).astype(np.float32)
+    mu_s = rng.uniform(2.0, 20.0, cfg.shape).astype(np.float32)
+    g = rng.uniform(0.7, 0.95, cfg.shape).astype(np.float32)
+    psi0 = wl.random_state(cfg, seed=7)
+    outs = []
+    for rep in range(2):
+        ctx = rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, dev(mu_a), dev(mu_s), dev(g), cfg.pml)
+        rte.rte_set_state(ctx, dev(psi0))
+        rte.rte_step(ctx, 3)
+        mid = gpu_state(ctx, cfg)
+        h = torch.empty((cfg.C,) + cfg.shape, dtype=torch.float32).pin_memory()
+        rte.rte_get_state_host(ctx, h)
+        assert np.array_equal(h.numpy().astype(np.float64), mid)
+        phi_h = torch.empty(cfg.shape, dtype=torch.float32).pin_memory()
+        rte.rte_fluence_host(ctx, phi_h)
+        assert np.array_equal(phi_h.numpy().astype(np.float64), mid[0])
+        rte.rte_step(ctx, 2)
+        outs.append((mid, gpu_state(ctx, cfg)))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_state(psi0)
+    o.step(3)
+    assert_parity(outs[0][0], o.get_state(), "double buffer, 3 steps")
+    o.step(2)
+    assert_parity(outs[0][1], o.get_state(), "double buffer, 5 steps")
+
+
 def test_fluence_change_steady_state_rule():
     """configs[3]'s stopping rule (R17): relative L2 change of the fluence over Omega between calls, against the same
     quantity computed from the oracle's fluence (dt = 0.02 ps is below the Euler bound of this medium, ~0.044 ps)."""
