@@ -329,6 +329,22 @@ def roofline_of(cfg, res, peak, peak_kind):
 TRAFFIC_NCU = {"cfg4": {0: 29698156000, 1: 43432037000, 2: 43430344000}}   # profiles/r1e_cfg4_pass_kernels.md
 
 
+def max_over_ranks(ms, dist, device):
+    """Device time of the job = the slowest rank's (replicas only: no data-path collective; this one scalar all-reduce
+    is the only communication, outside the timed region)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(cfg, steps, world, ms):
+    """Whole-job throughput: every rank advances its own replica of the workload (weak scaling)."""
+    return cfg.C * cfg.G * steps * world / (ms * 1e-3)
+
+
 def run_ours(args, wl, cfg):
     import torch
     try:
@@ -353,13 +369,9 @@ def run_ours(args, wl, cfg):
 
     sampler = ClockSampler(local) if rank == 0 else None
     res = measure_workload(rte, wl, cfg, torch, dev, args.steps, args.warmup, dist, sampler)
-    ms = res["ms"]
-    if dist is not None:      # max over ranks of the device time
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(res["ms"], dist, dev)
     units = cfg.C * cfg.G * args.steps * world
-    value = units / (ms * 1e-3)
+    value = job_value(cfg, args.steps, world, ms)
     ctx = res["ctx"]
 
     # ---- e2e: host buffers through the C ABI (pinned host -> device state, K steps, fluence device -> host) ----------
@@ -384,10 +396,7 @@ def run_ours(args, wl, cfg):
         torch.cuda.synchronize()
         wall_ms = 1e3 * (time.perf_counter() - t0)
         e_ms = max(e0.elapsed_time(e1), wall_ms)
-        if dist is not None:
-            t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
+        e_ms = max_over_ranks(e_ms, dist, dev)
         e2e = {"value": units / (e_ms * 1e-3), "unit": UNIT, "ms_total": e_ms,
                "h2d_bytes_per_step": h_state.numel() * 4 / args.steps, "d2h_bytes_per_step": h_phi.numel() * 4 / args.steps,
                "what": f"rte_set_state_host (pinned, {h_state.numel() * 4 / 1e9:.2f} GB) + {args.steps} x rte_step + rte_fluence_host, per rank"}
