@@ -7,7 +7,7 @@
 // permutation of the Cooley-Tukey split is a register renaming, i.e. free).
 //
 // Forward sign: X[k] = sum_j x[j] exp(-2 pi i j k / R)   (eq.(8): exp(-i k.r)).
-// Inverse (unnormalised) = swap(re,im) o forward o swap(re,im), also free of instructions.
+// Inverse (unnormalised): the same butterflies with conjugated twiddles (template flag INV).
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
@@ -117,16 +117,19 @@ RTE_HD float2 mulw(float2 a) {
 }
 
 // ---- DFT of R points held at v[0], v[S], v[2S], ...; natural order in and out --------------------------------------
-template <int R, int S>
+// INV = false: X[k] = sum_j x[j] exp(-2 pi i j k / R); INV = true: the unnormalised inverse, exp(+2 pi i j k / R) — the
+// same butterflies with every twiddle conjugated (no re/im swaps of the data, so results are born in the register
+// pairs the stores and reductions need).
+template <int R, int S, bool INV>
 struct Dft;
 
-template <int S>
-struct Dft<1, S> {
+template <int S, bool INV>
+struct Dft<1, S, INV> {
     static RTE_HD void run(float2*) {}
 };
 
-template <int S>
-struct Dft<2, S> {
+template <int S, bool INV>
+struct Dft<2, S, INV> {
     static RTE_HD void run(float2* v) {
         const float2 a = v[0], b = v[S];
         v[0] = cadd(a, b);
@@ -134,29 +137,29 @@ struct Dft<2, S> {
     }
 };
 
-template <int S>
-struct Dft<3, S> {
+template <int S, bool INV>
+struct Dft<3, S, INV> {
     static RTE_HD void run(float2* v) {
-        constexpr float hs3 = 0.86602540378443864676f;   // sqrt(3)/2
+        constexpr float hs3 = INV ? -0.86602540378443864676f : 0.86602540378443864676f;   // -+ sqrt(3)/2
         const float2 a = v[0], b = v[S], c = v[2 * S];
         const float2 s = cadd(b, c), d = csub(b, c);
         const float2 m = caxpy(-0.5f, s, a);
-        // X1 = m - i hs3 d ; X2 = m + i hs3 d
+        // forward: X1 = m - i hs3 d ; X2 = m + i hs3 d   (inverse: the conjugate twiddles swap the two)
         v[0] = cadd(a, s);
         v[S] = caxpy(hs3, make_float2(d.y, -d.x), m);
         v[2 * S] = caxpy(hs3, make_float2(-d.y, d.x), m);
     }
 };
 
-template <int S>
-struct Dft<4, S> {
+template <int S, bool INV>
+struct Dft<4, S, INV> {
     static RTE_HD void run(float2* v) {
         const float2 a = v[0], b = v[S], c = v[2 * S], d = v[3 * S];
         const float2 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = csub(b, d);
         v[0] = cadd(t0, t2);
         v[2 * S] = csub(t0, t2);
-        v[S] = cadd_mi(t1, t3);       // t1 - i t3
-        v[3 * S] = cadd_pi(t1, t3);   // t1 + i t3
+        v[S] = INV ? cadd_pi(t1, t3) : cadd_mi(t1, t3);       // t1 -+ i t3
+        v[3 * S] = INV ? cadd_mi(t1, t3) : cadd_pi(t1, t3);   // t1 +- i t3
     }
 };
 
@@ -167,21 +170,21 @@ struct Split {
     static constexpr int RB = R / RA;
 };
 
-template <int RA, int RB, int S, int KA, int B>
-struct TwiddleRow {   // v[(RB*KA + b)*S] *= W_R^{b*KA} for b = B..RB-1
+template <int RA, int RB, int S, int KA, int B, bool INV>
+struct TwiddleRow {   // v[(RB*KA + b)*S] *= W_R^{+-b*KA} for b = B..RB-1
     static RTE_HD void run(float2* v) {
         if constexpr (B < RB) {
-            v[(RB * KA + B) * S] = mulw<B * KA, RA * RB>(v[(RB * KA + B) * S]);
-            TwiddleRow<RA, RB, S, KA, B + 1>::run(v);
+            v[(RB * KA + B) * S] = mulw<(INV ? -B * KA : B * KA), RA * RB>(v[(RB * KA + B) * S]);
+            TwiddleRow<RA, RB, S, KA, B + 1, INV>::run(v);
         }
     }
 };
-template <int RA, int RB, int S, int KA>
+template <int RA, int RB, int S, int KA, bool INV>
 struct TwiddleAll {
     static RTE_HD void run(float2* v) {
         if constexpr (KA < RA) {
-            TwiddleRow<RA, RB, S, KA, 1>::run(v);
-            TwiddleAll<RA, RB, S, KA + 1>::run(v);
+            TwiddleRow<RA, RB, S, KA, 1, INV>::run(v);
+            TwiddleAll<RA, RB, S, KA + 1, INV>::run(v);
         }
     }
 };
@@ -191,15 +194,15 @@ struct TwiddleAll {
 //   step 2: slot (RB*ka + b) *= W_R^{b ka}
 //   step 3: for each ka, DFT_RB over b (stride S)             -> slot (RB*ka + kb) holds X[ka + RA*kb]
 //   step 4: un-permute (register renaming)
-template <int R, int S>
+template <int R, int S, bool INV>
 struct Dft {
     static constexpr int RA = Split<R>::RA, RB = Split<R>::RB;
     static RTE_HD void run(float2* v) {
 #pragma unroll
-        for (int b = 0; b < RB; ++b) Dft<RA, RB * S>::run(v + b * S);
-        TwiddleAll<RA, RB, S, 1>::run(v);
+        for (int b = 0; b < RB; ++b) Dft<RA, RB * S, INV>::run(v + b * S);
+        TwiddleAll<RA, RB, S, 1, INV>::run(v);
 #pragma unroll
-        for (int ka = 0; ka < RA; ++ka) Dft<RB, S>::run(v + ka * RB * S);
+        for (int ka = 0; ka < RA; ++ka) Dft<RB, S, INV>::run(v + ka * RB * S);
         float2 t[R];
 #pragma unroll
         for (int ka = 0; ka < RA; ++ka)
@@ -212,13 +215,21 @@ struct Dft {
 
 template <int R>
 RTE_HD void dft_fwd(float2 (&v)[R]) {
-    Dft<R, 1>::run(v);
+    Dft<R, 1, false>::run(v);
 }
 template <int R>
 RTE_HD void dft_inv(float2 (&v)[R]) {   // unnormalised inverse
+    Dft<R, 1, true>::run(v);
+}
+
+// The same inverse as swap(re,im) o forward o swap(re,im).  Needs two register moves per output when the result
+// feeds a store (the half-swap cannot fold into a store operand) but a few registers fewer than dft_inv; the x pass,
+// whose tail also holds the re-read psi column, uses it to stay spill-free at 128 registers.
+template <int R>
+RTE_HD void dft_inv_swap(float2 (&v)[R]) {
 #pragma unroll
     for (int i = 0; i < R; ++i) { const float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
-    Dft<R, 1>::run(v);
+    Dft<R, 1, false>::run(v);
 #pragma unroll
     for (int i = 0; i < R; ++i) { const float t = v[i].x; v[i].x = v[i].y; v[i].y = t; }
 }

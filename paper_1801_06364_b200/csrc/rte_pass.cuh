@@ -356,16 +356,16 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     float2 v[N1];
 #pragma unroll
     for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
-    rtefft::dft_inv<N1>(v);
+    if (MODE == MODE_FIRST) rtefft::dft_inv_swap<N1>(v);      // register pressure: see rte_fft.cuh
+    else rtefft::dft_inv<N1>(v);
     float2* sp = A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
     if (MODE == MODE_FIRST) {
-        const int ncell1 = n * A.TP + 1;
-        const float* s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
-        const float* s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
+        constexpr int ncell1 = n * (QC / PC) + 1;
+        const int i0 = __ldg(A.deg + 2 * p) * ncell1 + t * n + b, i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
         const SourceRow src(A, pencil0 + t, p);
 #pragma unroll
         for (int a = 0; a < N1; ++a) {
-            float2 e = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], v[a]);
+            float2 e = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], r[a], v[a]);
             src.add(a * N2 + b, e);
             stg64(sp, stepB * a, e);
         }
