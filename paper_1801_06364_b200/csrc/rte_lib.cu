@@ -27,7 +27,7 @@ thread_local char g_create_error[256] = "";
 
 struct AxisTables {
     CplEntry* cpl = nullptr;
-    int n = 0, N1 = 0, N2 = 0, maxcnt = 0;
+    int n = 0, N1 = 0, N2 = 0, maxcnt = 0, npure = 0;   // npure: leading coupling slots with pure blocks (rte_tables.h)
 };
 
 }  // namespace
@@ -383,7 +383,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     A.P = P;
     for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
         if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
-            !(axis == c->grid.dim - 1 && c->grid.dim == 3 && T.maxcnt > 2)) {
+            !(axis == 2 && T.maxcnt > 2) && !(axis < 2 && T.npure < 2)) {
             L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
             break;
         }
@@ -708,6 +708,7 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
         const double mcdt = -(double)c * (double)dt * 6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n;
         std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE);
         T.maxcnt = 0;
+        T.npure = rtetab::pair_layout(grid->dim, N).npure[a];
         for (int p = 0; p < ctx->P; ++p) {
             const int cnt = (int)pe[p].size();
             if (cnt > rtepass::kMaxE) {

@@ -227,6 +227,11 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
         float2* col = tile + b * SI + t * ST + p;
         float2 v[N1];
         if (CF) {
+            // The specialised kernels are launched as (FIRST, E = 4) on the x axis, (ACC, E = 4) on the y axis and
+            // (ACC, E = 2) on the z axis; the pair layout guarantees 2 pure slots on x (diagonal blocks) and y
+            // (off-diagonal blocks) — rte_tables.h PairLayout::npure, checked by the host before it picks these kernels.
+            constexpr int NPURE = (E == 4) ? 2 : 0;
+            constexpr bool PURE_DIAG = MODE == MODE_FIRST;
             const float2* srow[E];
             float2 wd[E], ws[E];
 #pragma unroll
@@ -243,8 +248,9 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
                     const float2 d = srow[e][(a * N2) * SI];
-                    u = rtefft::cfma_diag(wd[e].x, wd[e].y, d, u);
-                    u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
+                    // slots [0, NPURE) hold purely diagonal (x pass) / purely off-diagonal (y pass) blocks: one packed FMA
+                    if (e >= NPURE || PURE_DIAG) u = rtefft::cfma_diag(wd[e].x, wd[e].y, d, u);
+                    if (e >= NPURE || !PURE_DIAG) u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
                 }
                 v[a] = u;
             }

@@ -191,6 +191,9 @@ struct PairLayout {
     std::vector<int> inv;                          // inv[position] = base pair
     std::vector<std::vector<int>> slots[3];        // slots[axis][position][e] = source POSITION, or -1 (unused)
     int cost0 = 0, cost = 0, ideal = 0;            // modelled wavefronts: base layout, chosen layout, conflict-free
+    // slots [0, npure[axis]) of EVERY pair hold entries whose 2x2 block is purely diagonal (x, z axes) / purely
+    // off-diagonal (y axis) or empty, so the kernels spend one packed FMA per element on them instead of two
+    int npure[3] = {0, 0, 0};
 };
 
 inline int layout_tp(int dim, int N) {   // pencils per tile assumed by the model (the specialised kernels' choice)
@@ -245,7 +248,7 @@ inline const PairLayout& pair_layout(int dim, int N) {
     L.P = P;
     // coupling structure in base pair indices, padded with -1 to E entries per axis
     int E[3] = {4, 4, 4};
-    std::vector<std::vector<int>> src[3];
+    std::vector<std::vector<int>> src[3], pure[3];
     for (int a = 0; a < naxes; ++a) {
         std::vector<std::vector<PairEntry>> pe;
         pair_coupling_of(dim, N, a, ext, pe);
@@ -253,11 +256,23 @@ inline const PairLayout& pair_layout(int dim, int N) {
         for (auto& v : pe) mx = v.size() > mx ? v.size() : mx;
         if (dim == 3 && a == 2 && mx <= 2) E[a] = 2;            // the z kernels read 2 entries (rte_lib.cu launch_spec)
         if ((int)mx > E[a]) E[a] = (int)mx;
+        // entries of the axis' pure kind (block diagonal on x and z, off-diagonal on y) go first; gaps count as pure
         src[a].assign(P, {});
+        pure[a].assign(P, {});
+        int np = E[a];
         for (int p = 0; p < P; ++p) {
-            for (auto& en : pe[p]) src[a][p].push_back(en.src);
-            while ((int)src[a][p].size() < E[a]) src[a][p].push_back(-1);
+            std::vector<int> first, rest;
+            for (auto& en : pe[p]) {
+                const bool diag_only = en.w01 == 0.f && en.w10 == 0.f, swap_only = en.w00 == 0.f && en.w11 == 0.f;
+                ((a == 1 ? swap_only : diag_only) ? first : rest).push_back(en.src);
+            }
+            const int npair = E[a] - (int)rest.size();          // pure entries + gaps of this pair
+            if (npair < np) np = npair;
+            for (int s : first) { src[a][p].push_back(s); pure[a][p].push_back(1); }
+            while ((int)src[a][p].size() + (int)rest.size() < E[a]) { src[a][p].push_back(-1); pure[a][p].push_back(1); }
+            for (int s : rest) { src[a][p].push_back(s); pure[a][p].push_back(0); }
         }
+        L.npure[a] = np < 0 ? 0 : np;
     }
     std::vector<int> pos(P), inv(P);
     for (int p = 0; p < P; ++p) pos[p] = inv[p] = p;
@@ -281,7 +296,7 @@ inline const PairLayout& pair_layout(int dim, int N) {
     const int iters = (P > 2 && P <= 40 && cur > L.ideal) ? 20000 : 0;   // larger records: base layout (generic kernels)
     for (int itn = 0; itn < iters && best > L.ideal; ++itn) {
         const bool swap_move = (next() & 1) && P > 2;
-        int i = 0, j = 0, a = 0, p = 0;
+        int i = 0, j = 0, a = 0, p = 0, oldpure_swap[2] = {0, 0};
         std::vector<int> old;
         if (swap_move) {
             i = 1 + (int)(next() % (uint32_t)(P - 1));
@@ -292,7 +307,13 @@ inline const PairLayout& pair_layout(int dim, int N) {
         } else {
             a = (int)(next() % (uint32_t)naxes); p = (int)(next() % (uint32_t)P);
             old = src[a][p];
-            for (int k = E[a] - 1; k > 0; --k) std::swap(src[a][p][k], src[a][p][next() % (uint32_t)(k + 1)]);
+            // swap two slots of this pair; an entry may enter the pure class [0, npure) only if it is pure
+            const int e1 = (int)(next() % (uint32_t)E[a]), e2 = (int)(next() % (uint32_t)E[a]);
+            const int lo = e1 < e2 ? e1 : e2, hi = e1 < e2 ? e2 : e1;
+            if (lo == hi || (lo < L.npure[a] && !pure[a][p][hi])) continue;
+            std::swap(src[a][p][lo], src[a][p][hi]);
+            std::swap(pure[a][p][lo], pure[a][p][hi]);
+            oldpure_swap[0] = lo; oldpure_swap[1] = hi;
         }
         int nax[3] = {cax[0], cax[1], cax[2]};
         for (int k = 0; k < naxes; ++k)
@@ -301,7 +322,7 @@ inline const PairLayout& pair_layout(int dim, int N) {
         const double u = (double)(next() & 0xFFFFFF) / 16777216.0;
         if (c <= cur || u < std::exp((double)(cur - c) / T)) { cur = c; for (int k = 0; k < 3; ++k) cax[k] = nax[k]; }
         else if (swap_move) { std::swap(pos[i], pos[j]); inv[pos[i]] = i; inv[pos[j]] = j; }
-        else src[a][p] = old;
+        else { src[a][p] = old; std::swap(pure[a][p][oldpure_swap[0]], pure[a][p][oldpure_swap[1]]); }
         T = T * 0.9995 > 0.05 ? T * 0.9995 : 0.05;
         if (cur < best) { best = cur; best_pos = pos; for (int k = 0; k < 3; ++k) best_src[k] = src[k]; }
     }
