@@ -326,7 +326,7 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {"cfg4": {0: 29698156000, 1: 43432037000, 2: 43430344000}}   # profiles/r1e_cfg4_pass_kernels.md
+TRAFFIC_NCU = {"cfg4": {0: 29695333000, 1: 43428661000, 2: 43432189000}}   # profiles/r1f_pass_kernels.md
 
 
 def max_over_ranks(ms, dist, device):
