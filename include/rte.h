@@ -84,7 +84,8 @@ int rte_coupling_table(int dim, int N, int axis, double* A_out_host);
  * Returns RTE_EINVAL for dim not in {2,3} or N < 1. */
 int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* cost_host);
 
-/* Bytes of device workspace rte_create needs for this grid and order (state, partial sums, coefficient maps). */
+/* Bytes of device workspace rte_create needs for this grid and order (two state buffers — the step reads one and
+ * accumulates the next state into the other, then they trade places — and three per-cell coefficient maps). */
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out);
 
 /* ---- life cycle ---------------------------------------------------------------------------------------------- */
@@ -123,8 +124,10 @@ int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, 
 
 /* ---- the hot path ---------------------------------------------------------------------------------------------- */
 
-/* Advance nsteps forward-Euler steps (eq.(11)); asynchronous on the stream.  One step = one pencil-FFT kernel per
- * axis (DFT -> i k -> IDFT -> coupling), the last one fused with scattering, PML, source and the integrator. */
+/* Advance nsteps forward-Euler steps (eq.(11)); asynchronous on the stream.  One step = one pencil-FFT
+ * kernel per axis (coupling -> DFT -> i k -> IDFT, eq.(6)-(10)): the x kernel also applies scattering, PML and source
+ * (eq.(9),(12)) and stores psi(1 - c dt sigma_l) + c dt q - c dt T_x into the second state buffer, the other axes add
+ * their -c dt T_a to it; the buffers then trade places.  Results are bit-reproducible from run to run. */
 int rte_step(rte_ctx* ctx, int nsteps);
 
 /* Same as rte_step, but brackets every per-axis kernel with CUDA events on the context's stream and returns the
