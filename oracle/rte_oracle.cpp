@@ -33,7 +33,9 @@
 //         mu_b = mu_lo + (mu_hi-mu_lo) (1-cos(pi delta))/2 ; in the PML sigma_l = mu_b for every l, q = 0;
 //   R14 the source is sampled at t_n.
 //
-// Parity pins for every function here live in tests/test_oracle_pins.py (P1..P12); none is "parity unpinned".
+// Parity pins for every function here live in tests/test_oracle_pins.py (P1..P13); none is "parity unpinned".
+// Besides the paper's forward Euler there is one NON-PAPER integrator, SSP-RK3, built from the same
+// Euler update; it is pinned by the stability polynomial of a single Fourier mode (P13).
 //
 // Coefficient order (external, = the C-ABI's):  3-D  c = l*l + l + m  (m>=0 -> a_l^m, m<0 -> b_l^|m|);
 //                                                2-D  c = 0 -> a_0, c = 2m-1 -> a_m, c = 2m -> b_m.
@@ -408,12 +410,14 @@ static void streaming_literal(const Oracle* o, std::vector<double>& T) {
         }
 }
 
-static void one_step(Oracle* o, int formulation) {
+// psi <- psi - c dt ( T + sigma_l psi ) + c dt q(t_src): one forward-Euler update of eq.(11) with the source sampled
+// at an explicit time (the plain step samples it at t_n, R14; the Runge-Kutta stages below at their stage times)
+static void euler_update(Oracle* o, int formulation, double t_src) {
     const int C = o->C; const long G = o->G;
     std::vector<double> T;
     if (formulation == 0) streaming_literal(o, T); else streaming_per_axis(o, T);
     const double cdt = o->c * o->dt;
-    const double ft = source_time(o, (double)o->step_count * o->dt);   // R14: q at t_n
+    const double ft = source_time(o, t_src);
     o->psi_new.resize((size_t)C * G);
     for (int c = 0; c < C; ++c) {
         const int l = o->L[c];
@@ -447,6 +451,31 @@ static void one_step(Oracle* o, int formulation) {
         }
     }
     o->psi.swap(o->psi_new);
+}
+
+static void one_step(Oracle* o, int formulation) {
+    euler_update(o, formulation, (double)o->step_count * o->dt);   // R14: q at t_n
+    o->step_count += 1;
+}
+
+// SURVEY §8(f2), NOT the paper's integrator (the paper uses forward Euler, eq.(11)): the three-stage, third-order
+// strong-stability-preserving Runge-Kutta scheme of Shu & Osher written as convex combinations of Euler updates
+// E(u; t) = u + dt F(u, t) of the same semi-discrete system eq.(9):
+//     u1      = E(u^n; t_n)
+//     u2      = 3/4 u^n + 1/4 E(u1; t_n + dt)
+//     u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2)
+// For u' = M u it gives u^{n+1} = (I + z + z^2/2 + z^3/6) u^n, z = dt M (pinned in tests/test_oracle_pins.py); its
+// stability region contains |Im z| <= sqrt(3), so the skew-adjoint streaming operator no longer needs the scattering
+// damping to be stable and dt can approach dx/c (R10).
+static void one_step_ssprk3(Oracle* o, int formulation) {
+    const size_t n = o->psi.size();
+    const double tn = (double)o->step_count * o->dt;
+    const std::vector<double> u0 = o->psi;
+    euler_update(o, formulation, tn);                                   // psi = u1
+    euler_update(o, formulation, tn + o->dt);                           // psi = E(u1)
+    for (size_t i = 0; i < n; ++i) o->psi[i] = 0.75 * u0[i] + 0.25 * o->psi[i];          // u2
+    euler_update(o, formulation, tn + 0.5 * o->dt);                     // psi = E(u2)
+    for (size_t i = 0; i < n; ++i) o->psi[i] = u0[i] / 3.0 + (2.0 / 3.0) * o->psi[i];    // u^{n+1}
     o->step_count += 1;
 }
 
@@ -630,6 +659,10 @@ int orc_set_source(void* h, const double* w, const double* S, const int* origin,
 void orc_step(void* h, int nsteps, int formulation) {
     Oracle* o = (Oracle*)h;
     for (int s = 0; s < nsteps; ++s) one_step(o, formulation);
+}
+void orc_step_ssprk3(void* h, int nsteps, int formulation) {
+    Oracle* o = (Oracle*)h;
+    for (int s = 0; s < nsteps; ++s) one_step_ssprk3(o, formulation);
 }
 double orc_time_ps(void* h) { Oracle* o = (Oracle*)h; return (double)o->step_count * o->dt; }
 

@@ -44,6 +44,7 @@ def lib():
         L.orc_set_source.restype = C.c_int
         L.orc_set_source.argtypes = [C.c_void_p, dp, dp, ip, ip, C.c_int, C.c_double, C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.orc_step_ssprk3.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_time_ps.restype = C.c_double
         L.orc_time_ps.argtypes = [C.c_void_p]
         L.orc_streaming.argtypes = [C.c_void_p, C.c_int, dp]
@@ -193,6 +194,10 @@ class Oracle:
 
     def step(self, nsteps=1, formulation=PER_AXIS):
         lib().orc_step(self.h, int(nsteps), int(formulation))
+
+    def step_ssprk3(self, nsteps=1, formulation=PER_AXIS):
+        """NOT the paper's integrator: three-stage SSP Runge-Kutta built from the Euler update."""
+        lib().orc_step_ssprk3(self.h, int(nsteps), int(formulation))
 
     def time_ps(self):
         return float(lib().orc_time_ps(self.h))

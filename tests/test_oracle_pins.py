@@ -594,3 +594,89 @@ def test_step_cell_matches_full_step():
     for (x, y, z) in [(0, 0, 0), (4, 3, 2), (11, 7, 5), (5, 4, 3), (1, 6, 0), (6, 4, 3)]:
         v = o2.step_cell(psi0, x, y, z)
         assert np.abs(v - full[:, z, y, x]).max() < 1e-12 * np.abs(psi0).max()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# P13 — SSP-RK3 (NOT the paper's integrator): stability polynomial, order, stage times, large steps
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim,N,n,form", [(3, 3, 8, orc.PER_AXIS), (2, 4, 12, orc.LITERAL)])
+def test_P13_ssprk3_single_mode_stability_polynomial(dim, N, n, form):
+    """For u' = M u the Shu-Osher scheme is u_{n+1} = (I + z + z^2/2 + z^3/6) u_n, z = dt M(k), with M(k) built
+    independently from quadrature (as in P4)."""
+    rng = np.random.default_rng(13 * dim + N)
+    dx, c, dt = 0.2, 0.3, 0.05
+    mu_a, mu_s, g = 0.02, 4.0, 0.8
+    nz = n if dim == 3 else 1
+    j = np.array([2, -1, 3][:dim] + [0] * (3 - dim))
+    kvec = 2 * np.pi * j / (n * dx)
+    C = orc.num_coeffs(dim, N)
+    v = rng.standard_normal(C) + 1j * rng.standard_normal(C)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(n), np.arange(n), indexing="ij")
+    phase = np.exp(1j * dx * (kvec[0] * x + kvec[1] * y + kvec[2] * z))
+    o = orc.Oracle(dim, n, n, nz, N, dx, dt, c, mu_a, mu_s, g)
+    o.set_state((v[:, None, None, None] * phase[None]).real)
+    steps = 7
+    o.step_ssprk3(steps, form)
+    Z = dt * mode_matrix(dim, N, kvec, mu_a, mu_s, g, c)
+    Pz = np.eye(C) + Z + Z @ Z / 2 + Z @ Z @ Z / 6
+    vn = np.linalg.matrix_power(Pz, steps) @ v
+    ex = (vn[:, None, None, None] * phase[None]).real
+    assert np.abs(o.get_state() - ex).max() < 1e-12 * np.abs(v).max()
+    assert abs(o.time_ps() - steps * dt) < 1e-12
+
+
+def test_P13_ssprk3_third_order_and_stable_where_euler_is_not():
+    """(i) error against the matrix exponential falls by ~8 when dt halves; (ii) with mu_s = 0 (no damping) and
+    dt = 0.5 dx/c forward Euler amplifies a high mode every step while SSP-RK3 does not (|P(i y)| <= 1 for |y| <= sqrt 3)."""
+    from scipy.linalg import expm
+    dim, N, n = 3, 3, 8
+    dx, c = 0.2, 0.3
+    kvec = 2 * np.pi * np.array([1, 2, -1]) / (n * dx)
+    C = orc.num_coeffs(dim, N)
+    rng = np.random.default_rng(5)
+    v = rng.standard_normal(C) + 1j * rng.standard_normal(C)
+    z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    phase = np.exp(1j * dx * (kvec[0] * x + kvec[1] * y + kvec[2] * z))
+    M = mode_matrix(dim, N, kvec, 0.02, 4.0, 0.8, c)
+    t = 0.4
+    ex = ((expm(M * t) @ v)[:, None, None, None] * phase[None]).real
+    errs = []
+    for steps in (8, 16):
+        o = orc.Oracle(dim, n, n, n, N, dx, t / steps, c, 0.02, 4.0, 0.8)
+        o.set_state((v[:, None, None, None] * phase[None]).real)
+        o.step_ssprk3(steps)
+        errs.append(np.abs(o.get_state() - ex).max())
+    assert 6.0 < errs[0] / errs[1] < 10.0
+    dt = 0.5 * dx / c
+    norms = {}
+    wgt = np.sqrt(2 * orc.degrees(dim, N) + 1.0)[:, None, None, None]     # streaming is skew-adjoint in this norm (P6)
+    for name in ("euler", "ssprk3"):
+        o = orc.Oracle(dim, n, n, n, N, dx, dt, c, 0.0, 0.0, 0.0)
+        o.set_state((v[:, None, None, None] * phase[None]).real)
+        n0 = np.linalg.norm(wgt * o.get_state())
+        (o.step if name == "euler" else o.step_ssprk3)(40)
+        norms[name] = np.linalg.norm(wgt * o.get_state()) / n0
+    assert norms["euler"] > 5.0 and norms["ssprk3"] <= 1.0 + 1e-9
+
+
+def test_P13_ssprk3_source_stage_times():
+    """Uniform medium, uniform isotropic source with Gaussian time profile, psi = 0 initially, no streaming (uniform
+    field): the scheme reduces to the scalar SSP-RK3 of y' = -a y + b f(t) with stages at t_n, t_n + dt, t_n + dt/2."""
+    n, N, dx, dt, c = 4, 1, 0.3, 0.5, 0.3
+    mu_a, mu_s, g = 0.4, 0.0, 0.0
+    t0, sig = 1.2, 0.9
+    o = orc.Oracle(3, n, n, n, N, dx, dt, c, mu_a, mu_s, g)
+    w = np.zeros(o.C); w[0] = 1.0
+    o.set_source(w, np.full((n, n, n), 2.5), (0, 0, 0), (n, n, n), 2, t0, sig)
+    o.set_state(np.zeros((o.C, n, n, n)))
+    f = lambda t: np.exp(-0.5 * ((t - t0) / sig) ** 2)
+    E = lambda yv, t: yv + dt * (-c * mu_a * yv + c * 2.5 * f(t))
+    yv = 0.0
+    for s in range(5):
+        tn = s * dt
+        u1 = E(yv, tn)
+        u2 = 0.75 * yv + 0.25 * E(u1, tn + dt)
+        yv = yv / 3 + 2 / 3 * E(u2, tn + dt / 2)
+    o.step_ssprk3(5)
+    got = o.get_state()
+    assert np.abs(got[0] - yv).max() < 1e-13 and np.abs(got[1:]).max() < 1e-15
