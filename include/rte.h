@@ -130,6 +130,16 @@ int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, 
  * their -c dt T_a to it; the buffers then trade places.  Results are bit-reproducible from run to run. */
 int rte_step(rte_ctx* ctx, int nsteps);
 
+/* NOT the paper's integrator (the paper uses forward Euler and names better integrators as future work,
+ * PAPER.md:109,195): nsteps steps of the three-stage, third-order strong-stability-preserving Runge-Kutta scheme
+ * (Shu-Osher form) built from the same Euler update E(u; t) = u + dt F(u, t) of eq.(9):
+ *   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2).
+ * Its stability region contains the imaginary axis up to sqrt(3), so dt may approach dx/c instead of the
+ * scattering-limited Euler bound (R10).  Three Euler updates (9 pass kernels in 3-D) and two state-wide
+ * axpby kernels per step; allocates one extra state buffer (library-owned) on first use: RTE_ENOMEM if that fails.
+ * Asynchronous on the stream; rte_time_ps advances by dt per step. */
+int rte_step_ssprk3(rte_ctx* ctx, int nsteps);
+
 /* Same as rte_step, but brackets every per-axis kernel with CUDA events on the context's stream and returns the
  * accumulated device time per axis in milliseconds (ms_axis_host[3], host; unused axes get 0) and the number of
  * launches per axis actually timed (may be NULL).  Synchronises the stream before returning. */

@@ -57,6 +57,7 @@ _lib.rte_reset_time.argtypes = [_vp]
 _lib.rte_set_source.argtypes = [_vp, C.POINTER(C.c_float), _vp, _i3, _i3, _i, _f, _f]
 _lib.rte_set_source_host.argtypes = [_vp, C.POINTER(C.c_float), _vp, _i3, _i3, _i, _f, _f]
 _lib.rte_step.argtypes = [_vp, _i]
+_lib.rte_step_ssprk3.argtypes = [_vp, _i]
 _lib.rte_step_profile.argtypes = [_vp, _i, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
 _lib.rte_fluence_change.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rte_time_ps.argtypes = [_vp, C.POINTER(C.c_double)]
@@ -71,7 +72,7 @@ _lib.rte_pml_profile.argtypes = [C.POINTER(rte_grid), C.POINTER(rte_pml), _vp, _
 
 EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_workspace_bytes", "rte_create", "rte_destroy",
             "rte_set_state", "rte_get_state", "rte_set_state_host", "rte_get_state_host", "rte_reset_time",
-            "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_profile", "rte_fluence", "rte_fluence_host",
+            "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_ssprk3", "rte_step_profile", "rte_fluence", "rte_fluence_host",
             "rte_fluence_change", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
             "rte_media_ellipsoids", "rte_media_lognormal", "rte_pml_profile"]
 
@@ -238,6 +239,11 @@ def rte_set_source_host(ctx, w, S_host, box_origin, box_extent, temporal_kind, t
 
 def rte_step(ctx, nsteps=1):
     _check(_lib.rte_step(ctx.handle, int(nsteps)), ctx.handle)
+
+
+def rte_step_ssprk3(ctx, nsteps=1):
+    """NOT the paper's integrator: SSP-RK3 built from the Euler update (include/rte.h)."""
+    _check(_lib.rte_step_ssprk3(ctx.handle, int(nsteps)), ctx.handle)
 
 
 def rte_step_profile(ctx, nsteps=1):

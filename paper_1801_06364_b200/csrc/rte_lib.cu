@@ -50,6 +50,7 @@ struct rte_ctx {
     float* srcw = nullptr;
     float* srcS = nullptr;
     size_t srcS_cap = 0;
+    float2* extra = nullptr;       // third state buffer, library-owned, allocated by the first rte_step_ssprk3
     float* phi_prev = nullptr;
     double* red = nullptr;         // 2 doubles for reductions
     bool have_prev = false;
@@ -460,11 +461,12 @@ double source_time_factor(const rte_ctx* c, double t) {
     return 0.0;
 }
 
-int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
+// One forward-Euler update of eq.(11): out = in - c dt ( T[in] + sigma_l in ) + c dt q(t_src) — one pass kernel per axis.
+int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, cudaEvent_t* ev = nullptr) {
     const int naxes = c->grid.dim;
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
-        A.psi = c->psi; A.acc = c->part;
+        A.psi = in; A.acc = out;
         A.cpl = c->ax[axis].cpl;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
         A.cdt = c->c * c->dt; A.nsig = c->N + 1;
@@ -477,7 +479,7 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
         cudaError_t e;
         if (axis == 0) {
             if (c->src_kind != 0)
-                A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, (double)c->steps * (double)c->dt));
+                A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src));
             e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream)
                             : launch_generic<rtepass::MODE_FIRST>(n, A, L, c->stream);
         } else if (axis == 2) {
@@ -492,8 +494,56 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
         c->launches += 1;
         if (ev) cudaEventRecord(ev[axis], c->stream);
     }
-    // the accumulator now holds psi^{n+1}: the two state buffers trade places
+    return RTE_OK;
+}
+
+// the paper's step: psi^{n+1} = Euler update of psi^n with the source at t_n (R14); the two state buffers trade places
+int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
+    const int rc = euler_update(c, c->psi, c->part, (double)c->steps * (double)c->dt, ev);
+    if (rc != RTE_OK) return rc;
     std::swap(c->psi, c->part);
+    c->steps += 1;
+    return RTE_OK;
+}
+
+// y = a x + b y over a whole state buffer (the convex combinations of the Runge-Kutta stages)
+__global__ void k_axpby(float4* __restrict__ y, const float4* __restrict__ x, float a, float b, size_t n4) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        const float4 xv = x[i];
+        float4 yv = y[i];
+        yv.x = fmaf(a, xv.x, b * yv.x); yv.y = fmaf(a, xv.y, b * yv.y);
+        yv.z = fmaf(a, xv.z, b * yv.z); yv.w = fmaf(a, xv.w, b * yv.w);
+        y[i] = yv;
+    }
+}
+
+// SSP-RK3 (Shu-Osher form, not the paper's integrator):
+//   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2)
+int one_step_ssprk3(rte_ctx* c) {
+    const size_t field = align_up((size_t)c->G * c->Cp * sizeof(float), 256);
+    if (!c->extra) {
+        if (cudaMalloc((void**)&c->extra, field) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(c, RTE_ENOMEM, "rte_step_ssprk3 needs a third state buffer and the device is out of memory");
+        }
+    }
+    float2 *X = c->psi, *Y = c->part, *Z = c->extra;
+    const double tn = (double)c->steps * (double)c->dt, dt = (double)c->dt;
+    const size_t n4 = (size_t)c->G * c->Cp / 4;            // Cp is even and records are 8-byte pairs: G*Cp*4 B, /16
+    const size_t rem = ((size_t)c->G * c->Cp) % 4;
+    if (rem != 0) return fail(c, RTE_EUNSUPPORTED, "state size not a multiple of 16 bytes");
+    const int gb = grid_for((long long)n4, 256);
+    int rc = euler_update(c, X, Y, tn);
+    if (rc != RTE_OK) return rc;
+    rc = euler_update(c, Y, Z, tn + dt);
+    if (rc != RTE_OK) return rc;
+    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Z, (const float4*)X, 0.75f, 0.25f, n4);
+    rc = euler_update(c, Z, Y, tn + 0.5 * dt);
+    if (rc != RTE_OK) return rc;
+    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Y, (const float4*)X, (float)(1.0 / 3.0), (float)(2.0 / 3.0), n4);
+    c->launches += 2;
+    if (cudaGetLastError() != cudaSuccess) return fail(c, RTE_ECUDA, "CUDA: %s", "axpby launch failed");
+    c->psi = Y; c->part = X;                                // X (u^n) is free now; Z stays the spare buffer
     c->steps += 1;
     return RTE_OK;
 }
@@ -536,6 +586,7 @@ void free_ctx(rte_ctx* c) {
     for (int a = 0; a < 3; ++a) {
         cudaFree(c->ax[a].cpl);
     }
+    cudaFree(c->extra);
     cudaFree(c->deg); cudaFree(c->ext_of_slot); cudaFree(c->srcw); cudaFree(c->srcS); cudaFree(c->phi_prev);
     cudaFree(c->red);
     delete c;
@@ -814,6 +865,16 @@ int rte_step(rte_ctx* ctx, int nsteps) {
     if (nsteps < 0) return fail(ctx, RTE_EINVAL, "negative step count");
     for (int s = 0; s < nsteps; ++s) {
         const int rc = one_step(ctx);
+        if (rc != RTE_OK) return rc;
+    }
+    return RTE_OK;
+}
+
+int rte_step_ssprk3(rte_ctx* ctx, int nsteps) {
+    if (!ctx) return RTE_ESTATE;
+    if (nsteps < 0) return fail(ctx, RTE_EINVAL, "negative step count");
+    for (int s = 0; s < nsteps; ++s) {
+        const int rc = one_step_ssprk3(ctx);
         if (rc != RTE_OK) return rc;
     }
     return RTE_OK;
