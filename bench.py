@@ -36,11 +36,14 @@ if ROOT not in sys.path:
 METRIC = "coefficient-cell updates/s"
 UNIT = "coefficient-cells/s"
 DEFAULT_WORKLOAD = "cfg4"          # largest single-GPU configuration of BASELINE.json (384^3, P_7, 14.5 GB state)
-DEFAULT_STEPS = {"cfg0": 2000, "cfg1": 400, "cfg2": 400, "cfg3": 60, "cfg4": 40}
+DEFAULT_STEPS = {"cfg0": 2000, "cfg1": 400, "cfg2": 400, "cfg3": 60, "cfg4": 40,
+                 "paper_exp1": 400, "paper_exp2": 25000}       # the paper's own step counts
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # bounded oracle sample per workload: (grid extent, PML width, steps) — ~10-30 s of CPU work on ~8-32 cores
 ORACLE_SAMPLE = {"cfg0": (64, 0, 200), "cfg1": (256, 16, 6), "cfg2": (64, 8, 4), "cfg3": (64, 8, 2),
-                 "cfg4": (96, 8, 2)}
+                 "cfg4": (96, 8, 2), "paper_exp1": (32, 0, 3), "paper_exp2": (64, 9, 12)}
+# the paper's wall-clock for its two runs on a Tesla K40 (context, not the target): seconds for all steps
+PAPER_WALL_S = {"paper_exp1": (70.0, "PAPER.md:141"), "paper_exp2": (223.0, "PAPER.md:167")}
 
 
 def parse_args(argv=None):
@@ -48,7 +51,8 @@ def parse_args(argv=None):
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD,
+                    choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "paper_exp1", "paper_exp2"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
@@ -216,6 +220,8 @@ def device_media(rte, wl, cfg, torch, dev):
     """Media maps generated ON THE DEVICE by the geometry layer (north_star item (3)); scalars for homogeneous."""
     if cfg.media == "homogeneous":
         return cfg.background
+    if cfg.media == "slab":         # the paper's sharp mu_s step (exp. 1): a tiny host-made map
+        return tuple(torch.from_numpy(m).to(dev) for m in wl.media_maps(cfg))
     if cfg.media in ("disks", "ellipsoids"):
         a, s, g = (torch.empty(cfg.shape, dtype=torch.float32, device=dev) for _ in range(3))
         rte.rte_media_ellipsoids(cfg.grid, cfg.dx, cfg.background, wl.inclusion_list(cfg), a, s, g)
@@ -422,6 +428,12 @@ def run_ours(args, wl, cfg):
             "roofline": roof,
             "paper_context": {"k40_updates_per_s_complex": [7.25e8, 1.88e9], "source": "PAPER.md:141,167 (Tesla K40; context only)"}}
 
+    if cfg.name in PAPER_WALL_S:
+        k40_s, where = PAPER_WALL_S[cfg.name]
+        line["paper_run"] = {"steps": cfg.steps, "this_run_seconds_for_those_steps": ms / args.steps * cfg.steps * 1e-3,
+                             "paper_seconds_tesla_k40": k40_s, "source": where,
+                             "note": "the paper's own parameter set; its hardware, precision unstated: context only"}
+
     if not args.no_others and world == 1:
         # side measurement (not the paper's integrator): SSP-RK3 = 3 Euler updates + 2 axpby per step
         k = max(2, args.steps // 8)
@@ -469,7 +481,7 @@ def run_ours(args, wl, cfg):
 def main(argv=None):
     args = parse_args(argv)
     import rte_workloads as wl
-    cfg = wl.CONFIGS[args.workload]
+    cfg = wl.CONFIGS[args.workload] if args.workload in wl.CONFIGS else wl.PAPER_EXPERIMENTS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl, cfg)
     return run_ours(args, wl, cfg)

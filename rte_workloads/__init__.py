@@ -64,6 +64,23 @@ CONFIGS = {
 }
 
 
+# The paper's own two runs, as workloads: like-for-like wall-clock beside
+# the Tesla-K40 timings the paper prints (70 s / 223 s).  No expected output exists (Figures 1-4 carry no numbers).
+#   exp1: 50 mm cube, 64^3, P_21, mu_a 0.01, mu_s 1.0 (5.0 for x <= 15 mm), g 0.9, dt 0.1 ps, 400 steps, no PML,
+#         isotropic Gaussian initial radiance of 1/e diameter 1.5 mm (sigma = D / (2 sqrt 2)) at the centre.
+#   exp2: 35.5 mm real cube inside the 50 mm / 64^3 domain (PML of 9 cells, half-cosine 0.01 -> 1.0 mm^-1), P_7,
+#         mu_a 0.01, mu_s 10, g 0.95, dt 0.04 ps, 25 000 steps, constant isotropic Gaussian source (same width) offset
+#         8 mm in x from the centre.
+PAPER_EXPERIMENTS = {
+    "paper_exp1": Config("paper_exp1", 3, 64, 64, 64, 21, 50.0 / 64, 0.1, 0.3, 400, (0, 0.0, 0.0), "slab",
+                         "gaussian_pulse_ic", 0, background=(0.01, 1.0, 0.9),
+                         extra={"sigma_mm": 1.5 / (2.0 * math.sqrt(2.0)), "slab_mu_s": 5.0, "slab_x_mm": 15.0}),
+    "paper_exp2": Config("paper_exp2", 3, 64, 64, 64, 7, 50.0 / 64, 0.04, 0.3, 25000, (9, 0.01, 1.0), "homogeneous",
+                         "gaussian_constant_offset", 0, background=(0.01, 10.0, 0.95),
+                         extra={"sigma_mm": 1.5 / (2.0 * math.sqrt(2.0)), "offset_x_mm": 8.0}),
+}
+
+
 def reduced(cfg: Config, n: int, steps=None, pml_width=None, dt=None, dx=None) -> Config:
     """Same structure on an n^d grid (for parity runs the fp64 oracle can finish)."""
     W = cfg.pml[0] if pml_width is None else pml_width
@@ -184,6 +201,11 @@ def media_maps(cfg: Config):
         return tuple(np.full(cfg.shape, v, dtype=np.float32) for v in cfg.background)
     if cfg.media in ("disks", "ellipsoids"):
         return rasterize_inclusions(cfg, inclusion_list(cfg))
+    if cfg.media == "slab":       # the paper's sharp mu_s step: cells whose x, measured from the domain edge, is <= slab_x
+        mu_a, mu_s, g = (np.full(cfg.shape, v, dtype=np.float32) for v in cfg.background)
+        x_from_edge = np.arange(cfg.nx) * cfg.dx
+        mu_s[:, :, x_from_edge <= cfg.extra["slab_x_mm"]] = cfg.extra["slab_mu_s"]
+        return mu_a, mu_s, g
     if cfg.media == "lognormal":
         mu_a = np.full(cfg.shape, cfg.background[0], dtype=np.float32)
         g = np.full(cfg.shape, cfg.background[2], dtype=np.float32)
@@ -262,6 +284,11 @@ def source_term(cfg: Config):
         S, org, ext = gaussian_footprint(cfg, centre, cfg.extra["sigma_mm"])
         sig_t = cfg.extra["fwhm_ps"] / (2.0 * math.sqrt(2.0 * math.log(2.0)))
         return dict(w=isotropic_weights(cfg), S=S, origin=org, extent=ext, kind=2, t0=cfg.extra["t0_ps"], sigma_t=sig_t)
+    if cfg.source == "gaussian_constant_offset":
+        # constant isotropic Gaussian source, offset along +x from the centre
+        centre = (cfg.nx // 2 + int(round(cfg.extra["offset_x_mm"] / cfg.dx)), cfg.ny // 2, cfg.nz // 2)
+        S, org, ext = gaussian_footprint(cfg, centre, cfg.extra["sigma_mm"])
+        return dict(w=isotropic_weights(cfg), S=S, origin=org, extent=ext, kind=1, t0=0.0, sigma_t=1.0)
     if cfg.source == "collimated_constant":
         # +z collimated Gaussian disc on the first Omega layer at the -z face
         centre = (cfg.nx // 2, cfg.ny // 2, W)

@@ -387,6 +387,26 @@ def test_double_buffer_odd_steps_and_determinism(grid, N):
     assert_parity(outs[0][1], o.get_state(), "double buffer, 5 steps")
 
 
+def test_paper_experiment_2_first_steps():
+    """the paper's second run (64^3, P_7, PML, constant offset Gaussian source,
+    dt = 0.04 ps) at full size for its first 25 of 25 000 steps, against the oracle."""
+    cfg = wl.replace(wl.PAPER_EXPERIMENTS["paper_exp2"], steps=25)
+    got, ref, _ = run_both(cfg, *wl.media_maps(cfg), wl.initial_state(cfg), wl.source_term(cfg), cfg.steps)
+    assert np.abs(ref[0]).max() > 0
+    assert_parity(got, ref, "paper exp. 2")
+
+
+def test_paper_experiment_1_structure_reduced():
+    """the paper's first run (P_21 = 484 coefficients, sharp mu_s slab, Gaussian
+    initial radiance, dt = 0.1 ps) on a 32^3 grid with the same dx for 6 steps (the oracle needs ~1 s per step here)."""
+    base = wl.PAPER_EXPERIMENTS["paper_exp1"]
+    cfg = wl.reduced(base, 32, steps=6)
+    mu = wl.media_maps(cfg)
+    assert mu[1].max() == 5.0 and mu[1].min() == 1.0
+    got, ref, _ = run_both(cfg, *mu, wl.initial_state(cfg), None, cfg.steps)
+    assert_parity(got, ref, "paper exp. 1 (32^3)")
+
+
 @pytest.mark.parametrize("dim,n,N", [(3, 32, 3), (2, 64, 4), (3, 128, 3)])
 def test_ssprk3_against_oracle(dim, n, N):
     """SURVEY 8(f2) (NOT the paper's integrator): rte_step_ssprk3 vs the oracle's SSP-RK3 on heterogeneous media with a
