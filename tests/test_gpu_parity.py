@@ -444,6 +444,43 @@ def test_ssprk3_against_oracle(dim, n, N):
     assert_parity(gpu_state(ctx, cfg), o.get_state(), "euler after ssprk3")
 
 
+def test_steady_state_by_ssprk3_is_a_fixed_point_of_the_paper_step():
+    """configs[3]'s steady state, reached with the non-paper SSP-RK3 step at dt = 0.3 dx/c and the R17 stopping rule, must
+    be a fixed point of the PAPER's forward-Euler map: one oracle Euler step (small stable dt) of the converged GPU state
+    changes it by no more than the residual the stopping rule allows."""
+    n, N, dx, c = 32, 3, 0.2, 0.3
+    dt_rk = 0.3 * dx / c
+    cfg = wl.Config("ss3d", 3, n, n, n, N, dx, dt_rk, c, 0, (4, 0.05, 3.0), "homogeneous", "none", 0)
+    mu_a, mu_s, g = 0.05, 4.0, 0.8
+    w = wl.collimated_weights(cfg)
+    S = np.zeros((1, 5, 5), dtype=np.float32)
+    S[0, 2, 2] = 1.0 / dx ** 3
+    S[0, 1:4, 1:4] += 0.2 / dx ** 3
+    org, ext = (14, 14, 5), (5, 5, 1)
+    ctx = rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, mu_a, mu_s, g, cfg.pml)
+    rte.rte_set_source(ctx, w, dev(S), org, ext, 1)
+    rte.rte_fluence_change(ctx)
+    steps, change = 0, float("inf")
+    while steps < 6000 and not change < 1e-6:
+        rte.rte_step_ssprk3(ctx, 100)
+        steps += 100
+        change = rte.rte_fluence_change(ctx)
+    assert change < 1e-6, f"no steady state after {steps} steps (change {change:.2e})"
+    star = gpu_state(ctx, cfg)
+    assert np.isfinite(star).all() and np.abs(star[0]).max() > 0
+    dt_e = 0.002                                            # stable forward-Euler step of this medium
+    o = orc.Oracle(3, n, n, n, N, dx, dt_e, c, np.full(cfg.shape, mu_a), np.full(cfg.shape, mu_s), np.full(cfg.shape, g),
+                   *cfg.pml)
+    o.set_source(w, S, org, ext, 1)
+    o.set_state(star)
+    o.step(1)
+    after = o.get_state()
+    # d psi/dt at the converged state, relative to the state, per unit time: the RK run's own rate was
+    # change / (100 dt_rk) ~ 5e-8 / ps for the fluence; allow a generous multiple (fp32 state, all coefficients)
+    rate = np.linalg.norm(after[0] - star[0]) / np.linalg.norm(star[0]) / dt_e
+    assert rate < 1e-5, f"converged state is not a fixed point of the Euler map: relative rate {rate:.2e} per ps"
+
+
 def test_fluence_change_steady_state_rule():
     """configs[3]'s stopping rule (R17): relative L2 change of the fluence over Omega between calls, against the same
     quantity computed from the oracle's fluence (dt = 0.02 ps is below the Euler bound of this medium, ~0.044 ps)."""
