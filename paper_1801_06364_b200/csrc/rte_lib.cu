@@ -359,6 +359,7 @@ constexpr SpecRow kSpec[] = {
     {128, 8, 4, 256},    // cfg2: 128^3 P_3
     {512, 8, 2, 256},    // cfg1: 512^2 P_7 (2-D)
     {64, 4, 8, 256},     // cfg0: 64^2 P_3 (2-D)
+    {64, 32, 1, 256},    // the paper's second run: 64^3 P_7
 };
 
 size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
@@ -451,6 +452,7 @@ cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaSt
         case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, 3>(A, L, s);
         case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2>(A, L, s);
         case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3>(A, L, s);
+        case 5: return launch_one<8, 8, MODE, E, 32, 32, 256, 3>(A, L, s);
         default: return cudaErrorInvalidValue;
     }
 }
