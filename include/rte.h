@@ -24,6 +24,7 @@
  *   field layout     external arrays are [c][z][y][x] fp32, contiguous (x fastest).
  *   pointers         "_dev" arguments are CUDA device pointers (e.g. torch.Tensor.data_ptr()) valid on the context's
  *                    device; "_host" arguments are host pointers (pinned memory makes the copies asynchronous).
+ *                    Every call on a context must be made with the CUDA device that was current at rte_create.
  *                    The library never frees caller memory.  It keeps the workspace and the stream until
  *                    rte_destroy; every other array is consumed (stream-ordered) during the call.
  *   stream           all work is enqueued on the cudaStream_t passed to rte_create (NULL = legacy default

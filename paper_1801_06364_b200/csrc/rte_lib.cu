@@ -416,11 +416,15 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+    // the dynamic shared-memory limit is a per-device function attribute: set it once per (kernel instance, device)
+    static bool configured[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     kern<<<L.blocks, L.nt, L.smem, s>>>(A);
     return cudaGetLastError();
