@@ -57,6 +57,8 @@ struct PassArgs {
     const int* deg;         // [2P] degree l of every slot
     float cdt;              // c * dt
     int nsig;               // N + 1 degrees
+    float g_uniform;        // > 0: g is this number in every cell AND the kernel instance is a uniform-g one (UG): the
+                            // diagonal table then holds 2 numbers per cell (build_sig); 0: N+1 numbers per cell
     const float* srcS;      // [ext z][ext y][ext x], already zero outside Omega
     const float* srcw;      // [2P] angular weight per slot
     int src_org[3], src_ext[3];
@@ -325,10 +327,26 @@ __device__ __forceinline__ void phase_inv1(const PassArgs& A, float2* tile, int 
 // sigma_l = mu_a + mu_s (1 - g^l) in Omega (eq.(9); g^l by repeated multiplication, R16),
 //         = mu_b for every l in the PML, where the maps hold (mu_b, 0, g) (eq.(12)).
 // Layout sig[l*(ncell+1) + j], j = t*n + i: conflict-free to build (lanes = cells) and to read (lanes = degrees).
+// Uniform g (A.g_uniform > 0): s_l = 1 - c dt (sa + ss (1 - g^l)) = A + B g^l with A = 1 - c dt (sa + ss), B = c dt ss,
+// so the table holds the float2 (A, B) per cell and every thread keeps g^l of its two slots in registers: one
+// broadcast 8-byte read per element instead of two 4-byte reads, and a quarter of the table-building work.
 template <int N1, int N2>
 __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long long base, int valid, int tid, int nt) {
     constexpr int n = N1 * N2;
     const int ncell = n * A.TP;
+    if (A.g_uniform > 0.f) {
+        float2* ab = reinterpret_cast<float2*>(sig);
+        for (int j = tid; j < ncell; j += nt) {
+            const int t = j / n, i = j - t * n;
+            float sa = 0.f, ss = 0.f;
+            if (t < valid) {
+                const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
+                sa = __ldg(A.sa + cell); ss = __ldg(A.ss + cell);
+            }
+            ab[j] = make_float2(1.f - A.cdt * (sa + ss), A.cdt * ss);
+        }
+        return;
+    }
     for (int j = tid; j < ncell; j += nt) {
         const int t = j / n, i = j - t * n;
         float sa = 0.f, ss = 0.f, g = 0.f;
@@ -349,7 +367,7 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // ---- tail, specialised kernels: inverse first factor in registers, then one store / vector reduction per element ---------
 // (the coupling was applied in phase 1; every thread owns its column, so there is no barrier and no neighbour data)
 // FIRST: r holds the column's own psi (loaded by tail_load, the first task's before the phase-2 barrier).
-template <int N1, int N2, int MODE, int QC, int PC, bool STACKED>
+template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG>
 __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile, const float* sig, long long base, int task,
                                           long long pencil0, float2 (&r)[N1]) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
@@ -369,11 +387,25 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
         constexpr int ncell1 = n * (QC / PC) + 1;
         const int i0 = __ldg(A.deg + 2 * p) * ncell1 + t * n + b, i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
         const SourceRow src(A, pencil0 + t, p);
+        if (UG) {
+            const float2* ab = reinterpret_cast<const float2*>(sig) + t * n + b;
+            float g0 = 1.f, g1 = 1.f;
+            for (int l = __ldg(A.deg + 2 * p); l > 0; --l) g0 *= A.g_uniform;          // g^l by repeated multiplication (R16)
+            for (int l = __ldg(A.deg + 2 * p + 1); l > 0; --l) g1 *= A.g_uniform;
 #pragma unroll
-        for (int a = 0; a < N1; ++a) {
-            float2 e = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], r[a], v[a]);
-            src.add(a * N2 + b, e);
-            stg64(sp, stepB * a, e);
+            for (int a = 0; a < N1; ++a) {
+                const float2 c = ab[a * N2];
+                float2 e = rtefft::cfma_diag(fmaf(c.y, g0, c.x), fmaf(c.y, g1, c.x), r[a], v[a]);
+                src.add(a * N2 + b, e);
+                stg64(sp, stepB * a, e);
+            }
+        } else {
+#pragma unroll
+            for (int a = 0; a < N1; ++a) {
+                float2 e = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], r[a], v[a]);
+                src.add(a * N2 + b, e);
+                stg64(sp, stepB * a, e);
+            }
         }
     } else {
 #pragma unroll
@@ -448,7 +480,8 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
     for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
 }
 
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
+// UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
@@ -490,12 +523,12 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         // phase 2 (the loads depend on nothing in shared memory)
         if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
         __syncthreads();
-        tail_spec<N1, N2, MODE, QC, PC, STACKED>(A, tile, sig, base, tid, pencil0, r);
+        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
             if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
-            tail_spec<N1, N2, MODE, QC, PC, STACKED>(A, tile, sig, base, task, pencil0, r2);
+            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();
