@@ -465,8 +465,10 @@ template <int MODE, int E>
 cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     switch (spec) {
         case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2>(A, L, s);
-        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, 2>(A, L, s);
-        case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, 3>(A, L, s);
+        case 1: return MODE == rtepass::MODE_FIRST ? launch_one<16, 16, MODE, E, 36, 18, 288, 2>(A, L, s)
+                                                   : launch_one<16, 16, MODE, E, 36, 18, 288, 3>(A, L, s);
+        case 2: return MODE == rtepass::MODE_FIRST ? launch_one<16, 8, MODE, E, 32, 8, 256, 3>(A, L, s)
+                                                   : launch_one<16, 8, MODE, E, 32, 8, 256, 4>(A, L, s);
         case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2>(A, L, s);
         case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3>(A, L, s);
         case 5: return launch_one<8, 8, MODE, E, 32, 32, 256, 3>(A, L, s);
