@@ -25,7 +25,19 @@ def dev(a):
 
 
 def gpu_create(cfg, mu_a, mu_s, g):
-    return rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, dev(mu_a), dev(mu_s), dev(g), cfg.pml)
+    """Media as numpy maps (-> device maps) or python floats (-> 1-value device arrays: is_map = 0, which is what
+    bench.py passes for homogeneous workloads and what selects the uniform-g kernel instances)."""
+    m = [v if isinstance(v, float) else dev(v) for v in (mu_a, mu_s, g)]
+    return rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, m[0], m[1], m[2], cfg.pml)
+
+
+def media_of(cfg, kind):
+    """'maps': full fp32 maps from the CPU generators; 'scalars': the background as three python floats (homogeneous
+    configs only) — bench.py's launch configuration for cfg0 / cfg2 (bench.py device_media)."""
+    if kind == "maps":
+        return wl.media_maps(cfg)
+    assert cfg.media == "homogeneous"
+    return tuple(float(v) for v in cfg.background)
 
 
 def gpu_state(ctx, cfg):
@@ -133,10 +145,12 @@ def test_scalar_media_no_pml_no_source():
 # ---------------------------------------------------------------------------------------------------------------------
 # the five configs
 # ---------------------------------------------------------------------------------------------------------------------
-def test_cfg0_full():
-    """configs[0]: 2-D 64x64 P_3, homogeneous, periodic, Gaussian pulse, 200 steps — full size, full step count."""
+@pytest.mark.parametrize("media", ["maps", "scalars"])
+def test_cfg0_full(media):
+    """configs[0]: 2-D 64x64 P_3, homogeneous, periodic, Gaussian pulse, 200 steps — full size, full step count.
+    'scalars' is bench.py's launch configuration (uniform-g instance of the specialised x-pass kernel)."""
     cfg = wl.CONFIGS["cfg0"]
-    mu = wl.media_maps(cfg)
+    mu = media_of(cfg, media)
     got, ref, ctx = run_both(cfg, *mu, wl.initial_state(cfg), wl.source_term(cfg), cfg.steps)
     e, f = assert_parity(got, ref, "cfg0")
     # conservation-type sanity on the GPU result itself: total fluence decays as (1 - c dt mu_a)^n (P5/P3 combined)
@@ -164,22 +178,41 @@ def test_cfg1_full_size_40_steps():
     assert_parity(got, ref, "cfg1 full size")
 
 
-def test_cfg2_reduced_full_steps():
+@pytest.mark.parametrize("media", ["maps", "scalars"])
+def test_cfg2_reduced_full_steps(media):
     """configs[2] structure (P_3, homogeneous, PML, temporal-Gaussian face source) on 32^3, all 2000 steps."""
     cfg = wl.reduced(wl.CONFIGS["cfg2"], 32, pml_width=6)
-    mu = wl.media_maps(cfg)
+    mu = media_of(cfg, media)
     got, ref, _ = run_both(cfg, *mu, wl.initial_state(cfg), wl.source_term(cfg), 2000)
     assert_parity(got, ref, "cfg2@32")
     assert np.abs(ref[0]).max() > 0
 
 
-def test_cfg2_full_size_few_steps():
-    """configs[2] at 128^3 in bench.py's launch configuration: 4 whole oracle steps around the source peak."""
+@pytest.mark.parametrize("media", ["scalars", "maps"])
+def test_cfg2_full_size_few_steps(media):
+    """configs[2] at 128^3, 16-cell PML, temporal-Gaussian source: 4 whole oracle steps around the source peak from a
+    random state.  'scalars' passes mu_a, mu_s, g as single values exactly as bench.py does for this homogeneous
+    workload (bench.py device_media), i.e. the uniform-g instance pass_kernel<..., UG = true> of the x pass with its
+    2-number diagonal table — bench.py's launch configuration; 'maps' runs the g-map instance."""
     cfg = wl.CONFIGS["cfg2"]
     cfg = wl.replace(cfg, extra=dict(cfg.extra, t0_ps=0.2))
-    mu = wl.media_maps(cfg)
+    mu = media_of(cfg, media)
     got, ref, _ = run_both(cfg, *mu, wl.random_state(cfg, seed=2), wl.source_term(cfg), 4)
-    assert_parity(got, ref, "cfg2 full size")
+    assert_parity(got, ref, f"cfg2 full size ({media})")
+
+
+@pytest.mark.parametrize("name,n,N,W,steps", [("cfg0", 64, 3, 8, 50), ("cfg1", 512, 7, 16, 12)])
+def test_2d_uniform_g_instance_with_pml_and_source(name, n, N, W, steps):
+    """The uniform-g instances of the 2-D specialised x-pass kernels (64^2 P_3 and 512^2 P_7 tiles) with a PML and a
+    Gaussian-in-time box source, scalar media, from a random state (UG + PML + source had no oracle check)."""
+    base = wl.CONFIGS[name]
+    cfg = wl.replace(base, name=f"{name}-ug", media="homogeneous", pml=(W, 0.01, 4.0), steps=steps, n_inclusions=0)
+    rng = np.random.default_rng(n + N)
+    ext = (7, 5, 1)
+    src = dict(w=rng.standard_normal(cfg.C).astype(np.float32), S=rng.standard_normal(ext[::-1]).astype(np.float32),
+               origin=(W + 3, n - W - 9, 0), extent=ext, kind=2, t0=3.5 * cfg.dt, sigma_t=2.0 * cfg.dt)
+    got, ref, _ = run_both(cfg, *media_of(cfg, "scalars"), wl.random_state(cfg, seed=N), src, steps)
+    assert_parity(got, ref, f"{name} 2-D UG + PML + source")
 
 
 def test_cfg3_reduced():
@@ -200,9 +233,46 @@ def test_cfg4_reduced():
     assert_parity(got, ref, "cfg4@96")
 
 
+def structural_cells(cfg, mu, src, rng, n_surface=40):
+    """Cells a heterogeneous-media / PML / source bug would show up in first: the 8 corners, the 6 face centres, cells of
+    the outermost-but-one PML layer boundary (last PML cell next to Omega and first Omega cell) on every side at random
+    transverse positions, source-box cells, and cells on inclusion surfaces (where a medium map changes along x, y or z)."""
+    n = (cfg.nx, cfg.ny, cfg.nz)
+    W = cfg.pml[0]
+    cells = [(x, y, z) for x in (0, n[0] - 1) for y in (0, n[1] - 1) for z in (0, n[2] - 1)]
+    for a in range(3):
+        for v in (0, n[a] - 1):
+            c = [n[0] // 2, n[1] // 2, n[2] // 2]
+            c[a] = v
+            cells.append(tuple(c))
+    if W > 0:
+        for a in range(3):
+            for v in (W - 1, W, n[a] - 1 - W, n[a] - W):        # last PML cell | first Omega cell | last Omega | first PML
+                for _ in range(3):
+                    c = [int(rng.integers(W, n[k] - W)) for k in range(3)]
+                    c[a] = v
+                    cells.append(tuple(c))
+    if src is not None:
+        o, e = src["origin"], src["extent"]
+        for _ in range(8):
+            cells.append(tuple(int(o[k] + rng.integers(e[k])) for k in range(3)))
+        cells.append((o[0] + e[0] // 2, o[1] + e[1] // 2, o[2]))
+    for m in mu:                                               # inclusion / field surfaces
+        if isinstance(m, np.ndarray) and m.ndim == 3:
+            for axis in range(3):
+                d = np.diff(m, axis=axis) != 0
+                idx = np.argwhere(d)
+                if len(idx) == 0 or len(idx) > 0.5 * m.size:  # homogeneous, or a smooth field (every cell differs)
+                    continue
+                pick = idx[rng.choice(len(idx), size=min(n_surface // 3, len(idx)), replace=False)]
+                cells += [(int(x), int(y), int(z)) for z, y, x in pick]
+    return cells
+
+
 def sampled_full_size_check(cfg, mu, psi0, src, ncells, seed):
     """One step at full size in bench.py's launch configuration, checked on sampled cells the oracle computes one by
-    one (orc_step_cell: direct circulant sum along the three pencils through the cell)."""
+    one (orc_step_cell: direct circulant sum along the three pencils through the cell): ncells random cells plus the
+    structural ones (corners, faces, PML/Omega interface, source box, inclusion surfaces)."""
     mu_a, mu_s, g = mu
     ctx = gpu_create(cfg, mu_a, mu_s, g)
     rte.rte_set_state(ctx, dev(psi0))
@@ -216,22 +286,29 @@ def sampled_full_size_check(cfg, mu, psi0, src, ncells, seed):
     rte.rte_sync(ctx)
     rng = np.random.default_rng(seed)
     cells = [(int(rng.integers(cfg.nx)), int(rng.integers(cfg.ny)), int(rng.integers(cfg.nz))) for _ in range(ncells)]
-    if src is not None:   # make sure source cells, PML cells and corners are among the samples
-        ox, oy, oz = src["origin"]
-        cells += [(ox + src["extent"][0] // 2, oy + src["extent"][1] // 2, oz), (0, 0, 0), (cfg.nx - 1, cfg.ny // 2, cfg.nz - 1)]
+    cells += structural_cells(cfg, mu, src, rng)
+    ix = torch.tensor(cells, dtype=torch.long, device=DEV)
+    got_all = out[:, ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy().astype(np.float64)        # [C, ncells]
     scale = np.sqrt(np.mean(psi0.astype(np.float64) ** 2, axis=(1, 2, 3)))
     worst = 0.0
-    for (x, y, z) in cells:
+    for j, (x, y, z) in enumerate(cells):
         ref = o.step_cell(psi0, x, y, z)
-        got = out[:, z, y, x].cpu().numpy().astype(np.float64)
-        worst = max(worst, np.max(np.abs(got - ref) / np.maximum(np.abs(ref), scale)))
-    assert worst < 2e-5, f"{cfg.name}: sampled one-step error {worst:.3e}"
+        worst = max(worst, np.max(np.abs(got_all[:, j] - ref) / np.maximum(np.abs(ref), scale)))
+    assert len(cells) >= 200
+    assert worst < 2e-5, f"{cfg.name}: sampled one-step error {worst:.3e} over {len(cells)} cells"
 
 
 def test_cfg3_full_size_sampled():
     cfg = wl.CONFIGS["cfg3"]
     mu = wl.media_maps(cfg)
-    sampled_full_size_check(cfg, mu, wl.random_state(cfg, seed=3), wl.source_term(cfg), 24, 3)
+    sampled_full_size_check(cfg, mu, wl.random_state(cfg, seed=3), wl.source_term(cfg), 200, 3)
+
+
+def test_cfg2_full_size_sampled_scalar_media():
+    """cfg2 exactly as bench.py launches it (scalar media => UG instance, 16-cell PML, temporal source at its peak)."""
+    cfg = wl.CONFIGS["cfg2"]
+    cfg = wl.replace(cfg, extra=dict(cfg.extra, t0_ps=0.0))
+    sampled_full_size_check(cfg, media_of(cfg, "scalars"), wl.random_state(cfg, seed=2), wl.source_term(cfg), 200, 2)
 
 
 def host_ram_gb():
@@ -256,7 +333,7 @@ def test_cfg4_full_size_sampled():
     rte.rte_media_lognormal(cfg.grid, cfg.dx, cfg.seed, 10.0, cfg.extra["sigma_log"], cfg.extra["corr_len_mm"], mu_s_d, scratch)
     mu_s = mu_s_d.cpu().numpy()
     del scratch
-    sampled_full_size_check(cfg, (mu_a, mu_s, g), wl.random_state(cfg, seed=4), None, 12, 4)
+    sampled_full_size_check(cfg, (mu_a, mu_s, g), wl.random_state(cfg, seed=4), None, 200, 4)
 
 
 # ---------------------------------------------------------------------------------------------------------------------
@@ -394,6 +471,19 @@ def test_paper_experiment_2_first_steps():
     got, ref, _ = run_both(cfg, *wl.media_maps(cfg), wl.initial_state(cfg), wl.source_term(cfg), cfg.steps)
     assert np.abs(ref[0]).max() > 0
     assert_parity(got, ref, "paper exp. 2")
+
+
+def test_paper_experiment_1_full_size_two_steps():
+    """the paper's first run at its REAL size (64^3, P_21 = 484 coefficients, P = 242
+    pairs: the large-C generic kernels), 2 whole oracle steps from a random state on top of the Gaussian initial
+    radiance."""
+    cfg = wl.replace(wl.PAPER_EXPERIMENTS["paper_exp1"], steps=2)
+    if host_ram_gb() < 24:
+        pytest.skip("needs ~12 GB of host RAM for the fp64 oracle state and its streaming term")
+    mu = wl.media_maps(cfg)
+    psi0 = wl.initial_state(cfg) + 1e-3 * wl.random_state(cfg, seed=21, decay=0.8)
+    got, ref, _ = run_both(cfg, *mu, psi0.astype(np.float32), None, cfg.steps)
+    assert_parity(got, ref, "paper exp. 1 (64^3, P_21)")
 
 
 def test_paper_experiment_1_structure_reduced():

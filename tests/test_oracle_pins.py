@@ -202,6 +202,41 @@ def test_P2_wavenumbers():
 
 
 # ------------------------------------------------------------------------------------------------------------------
+# degrees(): which power of g each external coefficient takes in sigma = mu_a + mu_s (1 - g^l)  (eq.(5), PAPER.md:66-69;
+# 2-D: l == |m|, reading R8).  The expected side of P3 / P4 below uses THIS hand-written table, not orc.degrees.
+# ------------------------------------------------------------------------------------------------------------------
+def hand_degrees(dim, N):
+    """Written out from the coefficient order alone: 3-D c = l*l + l + m, m = -l..l  =>  2l+1 consecutive entries of l;
+    2-D c = 0 -> a_0, c = 2m-1 -> a_m, c = 2m -> b_m  =>  0, 1, 1, 2, 2, ..."""
+    if dim == 3:
+        return np.array([l for l in range(N + 1) for _ in range(2 * l + 1)])
+    return np.array([0] + [m for m in range(1, N + 1) for _ in (0, 1)])
+
+
+def test_degrees_tables_written_out():
+    assert list(orc.degrees(2, 3)) == [0, 1, 1, 2, 2, 3, 3]
+    assert list(orc.degrees(2, 1)) == [0, 1, 1]
+    assert list(orc.degrees(2, 7)) == [0, 1, 1, 2, 2, 3, 3, 4, 4, 5, 5, 6, 6, 7, 7]
+    assert list(orc.degrees(3, 2)) == [0, 1, 1, 1, 2, 2, 2, 2, 2]
+    assert list(orc.degrees(3, 3)) == [0] + [1] * 3 + [2] * 5 + [3] * 7
+
+
+def test_henyey_greenstein_eigenvalues_are_g_to_the_order():
+    """Why the diagonal is mu_s g^l (3-D, eq.(2),(5)) and mu_s g^|m| (2-D, R8): the Legendre /
+    Fourier coefficients of the phase function, by quadrature."""
+    g = 0.87
+    x, w = np.polynomial.legendre.leggauss(200)
+    p3 = (1 - g * g) / (4 * np.pi * (1 + g * g - 2 * g * x) ** 1.5)           # eq.(2)
+    for l in range(8):
+        Pl = np.polynomial.legendre.Legendre.basis(l)(x)
+        assert abs(2 * np.pi * np.sum(w * p3 * Pl) - g ** l) < 1e-12
+    th = 2 * np.pi * np.arange(4096) / 4096
+    p2 = (1 - g * g) / (2 * np.pi * (1 + g * g - 2 * g * np.cos(th)))         # 2-D Henyey-Greenstein kernel (R8)
+    for m in range(8):
+        assert abs(np.sum(p2 * np.cos(m * th)) * (2 * np.pi / 4096) - g ** m) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------------------------
 # P3 — uniform field decays as (1 - c dt sigma_l)^n -> exp(-c sigma_l t)  (sigma_l = mu_a + mu_s (1-g^l); R3, R4)
 # ------------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dim,N,form", [(3, 3, orc.PER_AXIS), (3, 2, orc.LITERAL), (2, 3, orc.PER_AXIS), (2, 3, orc.LITERAL)])
@@ -216,7 +251,7 @@ def test_P3_uniform_decay(dim, N, form):
     steps = 25
     o.step(steps, form)
     psi = o.get_state()
-    L = orc.degrees(dim, N)
+    L = hand_degrees(dim, N)                    # not orc.degrees: the expected side is independent of the oracle
     sigma = mu_a + mu_s * (1 - g ** L)
     ex = amp * (1 - c * dt * sigma) ** steps
     assert np.abs(psi - ex[:, None, None, None]).max() < 1e-13 * amp.max()
@@ -257,7 +292,7 @@ def test_P3_heterogeneous_maps_pointwise():
     o = orc.Oracle(3, nx, ny, nz, N, 0.1, dt, c, mu_a, mu_s, g)
     o.set_state(np.ones((o.C, nz, ny, nx)))
     o.step(1)
-    L = orc.degrees(3, N)
+    L = hand_degrees(3, N)
     ex = 1 - c * dt * (mu_a[None] + mu_s[None] * (1 - g[None] ** L[:, None, None, None]))
     assert np.abs(o.get_state() - ex).max() < 1e-14
 
@@ -267,7 +302,7 @@ def test_P3_heterogeneous_maps_pointwise():
 # ------------------------------------------------------------------------------------------------------------------
 def mode_matrix(dim, N, kvec, mu_a, mu_s, g, c):
     A = quad_coupling(dim, N)
-    L = orc.degrees(dim, N)
+    L = hand_degrees(dim, N)                    # not orc.degrees: M(k) is built without the oracle
     sigma = mu_a + mu_s * (1 - g ** L)
     M = -c * (1j * sum(kvec[a] * A[a] for a in range(dim)) + np.diag(sigma))
     return M
@@ -378,7 +413,7 @@ def test_P7_source_fixed_point(dim):
     w = np.arange(1, o.C + 1) * 0.25
     S = np.full((nz, n, n), 2.0)
     o.set_source(w, S, (0, 0, 0), (n, n, nz), 1)
-    L = orc.degrees(dim, 2)
+    L = hand_degrees(dim, 2)
     sigma = mu_a + mu_s * (1 - g ** L)
     fixed = 2.0 * w / sigma
     o.set_state(np.broadcast_to(fixed[:, None, None, None], (o.C, nz, n, n)))
@@ -505,7 +540,7 @@ def test_P10_scattering_switched_off_in_layer():
     o.set_state(np.ones((o.C, n, n, n)))
     o.step(1)
     mu_b, inside = orc.pml_map(3, n, n, n, W, 0.05, 2.0)
-    L = orc.degrees(3, N)
+    L = hand_degrees(3, N)
     sig_in = 0.05 + 8.0 * (1 - 0.9 ** L)
     ex = np.where(inside[None] == 1, 1 - c * dt * sig_in[:, None, None, None], 1 - c * dt * mu_b[None])
     assert np.abs(o.get_state() - ex).max() < 1e-15
