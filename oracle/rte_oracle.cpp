@@ -33,9 +33,11 @@
 //         mu_b = mu_lo + (mu_hi-mu_lo) (1-cos(pi delta))/2 ; in the PML sigma_l = mu_b for every l, q = 0;
 //   R14 the source is sampled at t_n.
 //
-// Parity pins for every function here live in tests/test_oracle_pins.py (P1..P13); none is "parity unpinned".
+// Parity pins for every function here live in tests/test_oracle_pins.py (P1..P16); none is "parity unpinned".
 // Besides the paper's forward Euler there is one NON-PAPER integrator, SSP-RK3, built from the same
-// Euler update; it is pinned by the stability polynomial of a single Fourier mode (P13).
+// Euler update; it is pinned by the stability polynomial of a single Fourier mode (P13).  SURVEY §8(f1)/(f2) add the
+// steady-state operator L = T + sigma_l (P14), a plain restarted GMRES on it (P15: dense solve, closed form, true
+// residual) and the exponential / integrating-factor Euler step (P16: exact uniform decay and source response).
 //
 // Coefficient order (external, = the C-ABI's):  3-D  c = l*l + l + m  (m>=0 -> a_l^m, m<0 -> b_l^|m|);
 //                                                2-D  c = 0 -> a_0, c = 2m-1 -> a_m, c = 2m -> b_m.
@@ -480,6 +482,153 @@ static void one_step_ssprk3(Oracle* o, int formulation) {
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// the steady-state operator, a Krylov solve with it, and the exponential (integrating-factor) step.
+// PAPER.md:109 ("...related to the method of exponential integrators.  Krylov subspace iterative methods can then be
+// employed to find a steady-state solution through repeated application of the implicit operator") and PAPER.md:195.
+// ------------------------------------------------------------------------------------------------------------
+// sigma_l(r) of eq.(9)/(12): mu_a + mu_s (1 - g^l) in Omega, mu_b in the layer
+static double sigma_of(const Oracle* o, int l, long r) {
+    if (!o->inside[r]) return o->mu_b[r];
+    double gl = 1.0;
+    for (int j = 0; j < l; ++j) gl *= o->g[r];
+    return o->mu_a[r] + o->mu_s[r] * (1.0 - gl);
+}
+
+// The time-independent transport operator of eq.(9) with d/dt = 0:   (L psi)_c = T_c[psi] + sigma_l psi_c,
+// so that eq.(9) reads  d psi/dt = -c L psi + c q  and a steady state satisfies  L psi = q.   y = L x, both [C][G].
+static void apply_operator(Oracle* o, int formulation, const std::vector<double>& x, std::vector<double>& y) {
+    const int C = o->C; const long G = o->G;
+    std::vector<double> keep = x;          // the streaming routines read o->psi
+    keep.swap(o->psi);
+    std::vector<double> T;
+    if (formulation == 0) streaming_literal(o, T); else streaming_per_axis(o, T);
+    y.resize((size_t)C * G);
+    for (int c = 0; c < C; ++c) {
+        const int l = o->L[c];
+#pragma omp parallel for schedule(static)
+        for (long r = 0; r < G; ++r) y[(size_t)c * G + r] = T[(size_t)c * G + r] + sigma_of(o, l, r) * o->psi[(size_t)c * G + r];
+    }
+    keep.swap(o->psi);
+}
+
+// q_c(r) = w_c S(r) 1_Omega(r): the spatial/angular part of the source (temporal factor 1), [C][G]
+static void source_field(const Oracle* o, std::vector<double>& q) {
+    const int C = o->C; const long G = o->G;
+    q.assign((size_t)C * G, 0.0);
+    if (o->src_kind == 0) return;
+    for (int c = 0; c < C; ++c)
+        for (int bz = 0; bz < o->src_ext[2]; ++bz)
+            for (int by = 0; by < o->src_ext[1]; ++by)
+                for (int bx = 0; bx < o->src_ext[0]; ++bx) {
+                    const int x = o->src_org[0] + bx, y = o->src_org[1] + by, z = o->src_org[2] + bz;
+                    const long r = ((long)z * o->ny + y) * o->nx + x;
+                    if (!o->inside[r]) continue;
+                    q[(size_t)c * G + r] = o->src_w[c] * o->src_S[((size_t)bz * o->src_ext[1] + by) * o->src_ext[0] + bx];
+                }
+}
+
+// Restarted GMRES(m) for L x = b (textbook: Saad, "Iterative methods for sparse linear systems", Alg. 6.9 — Arnoldi
+// with modified Gram-Schmidt, Givens rotations on the Hessenberg matrix), plain Euclidean inner product, no
+// preconditioner.  x holds the initial guess on entry and the solution on exit.  Stops when the TRUE residual
+// ||b - L x|| / ||b|| (recomputed at every restart) is <= tol or after max_restarts cycles.  Returns the number of
+// operator applications; *relres_out = the final true relative residual.
+static long gmres_solve(Oracle* o, int formulation, const std::vector<double>& b, std::vector<double>& x, int m,
+                        double tol, int max_restarts, double* relres_out) {
+    const size_t n = b.size();
+    auto dot = [&](const std::vector<double>& u, const std::vector<double>& v) {
+        double s = 0;
+#pragma omp parallel for reduction(+ : s) schedule(static)
+        for (long i = 0; i < (long)n; ++i) s += u[i] * v[i];
+        return s;
+    };
+    const double bnorm = std::sqrt(dot(b, b));
+    long applications = 0;
+    double relres = 0.0;
+    if (bnorm == 0.0) { x.assign(n, 0.0); *relres_out = 0.0; return 0; }
+    std::vector<std::vector<double>> V((size_t)m + 1);
+    std::vector<double> H((size_t)(m + 1) * m), cs(m), sn(m), gv(m + 1), w, r;
+    for (int cycle = 0; cycle <= max_restarts; ++cycle) {
+        apply_operator(o, formulation, x, w); ++applications;
+        r.resize(n);
+        for (size_t i = 0; i < n; ++i) r[i] = b[i] - w[i];
+        const double beta = std::sqrt(dot(r, r));
+        relres = beta / bnorm;
+        if (relres <= tol || cycle == max_restarts) break;
+        V[0].resize(n);
+        for (size_t i = 0; i < n; ++i) V[0][i] = r[i] / beta;
+        std::fill(gv.begin(), gv.end(), 0.0);
+        gv[0] = beta;
+        int k = 0;
+        for (; k < m; ++k) {
+            apply_operator(o, formulation, V[k], w); ++applications;
+            for (int j = 0; j <= k; ++j) {                       // modified Gram-Schmidt
+                const double h = dot(w, V[j]);
+                H[(size_t)j * m + k] = h;
+                for (size_t i = 0; i < n; ++i) w[i] -= h * V[j][i];
+            }
+            const double hn = std::sqrt(dot(w, w));
+            H[(size_t)(k + 1) * m + k] = hn;
+            for (int j = 0; j < k; ++j) {                        // earlier rotations on the new column
+                const double a = H[(size_t)j * m + k], c2 = H[(size_t)(j + 1) * m + k];
+                H[(size_t)j * m + k] = cs[j] * a + sn[j] * c2;
+                H[(size_t)(j + 1) * m + k] = -sn[j] * a + cs[j] * c2;
+            }
+            const double a = H[(size_t)k * m + k], d = std::sqrt(a * a + hn * hn);
+            cs[k] = a / d; sn[k] = hn / d;
+            H[(size_t)k * m + k] = d; H[(size_t)(k + 1) * m + k] = 0.0;
+            gv[k + 1] = -sn[k] * gv[k];
+            gv[k] = cs[k] * gv[k];
+            if (hn > 0) {
+                V[k + 1].resize(n);
+                for (size_t i = 0; i < n; ++i) V[k + 1][i] = w[i] / hn;
+            }
+            if (std::fabs(gv[k + 1]) / bnorm <= 0.1 * tol || hn == 0.0) { ++k; break; }
+        }
+        std::vector<double> yv(k);                               // back substitution  H y = g
+        for (int i = k - 1; i >= 0; --i) {
+            double s = gv[i];
+            for (int j = i + 1; j < k; ++j) s -= H[(size_t)i * m + j] * yv[j];
+            yv[i] = s / H[(size_t)i * m + i];
+        }
+        for (int j = 0; j < k; ++j)
+            for (size_t i = 0; i < n; ++i) x[i] += yv[j] * V[j][i];
+    }
+    *relres_out = relres;
+    return applications;
+}
+
+// Exponential (integrating-factor) Euler step — SURVEY §8(f2), the family PAPER.md:109 points to; NOT eq.(11).
+// The diagonal part of eq.(9), d psi/dt = -c sigma_l psi, is integrated exactly over the step and the streaming term
+// explicitly (Lawson / integrating-factor Euler); the source enters through phi_1 so that a constant source is also
+// integrated exactly where the streaming term vanishes:
+//     psi_{n+1} = E ( psi_n - c dt T[psi_n] ) + Phi c dt q(t_n),     E = exp(-c dt sigma_l),  Phi = (1 - E)/(c dt sigma_l)
+// (Phi = 1 where sigma_l = 0).  For a spatially uniform field (T = 0): psi(t_n) = e^{-c sigma_l t_n} psi(0)
+// + (q/sigma_l)(1 - e^{-c sigma_l t_n}) with no O(dt) error — the pin.
+static void one_step_exp(Oracle* o, int formulation) {
+    const int C = o->C; const long G = o->G;
+    std::vector<double> T;
+    if (formulation == 0) streaming_literal(o, T); else streaming_per_axis(o, T);
+    const double cdt = o->c * o->dt;
+    const double ft = source_time(o, (double)o->step_count * o->dt);
+    std::vector<double> q;
+    source_field(o, q);
+    o->psi_new.resize((size_t)C * G);
+    for (int c = 0; c < C; ++c) {
+        const int l = o->L[c];
+#pragma omp parallel for schedule(static)
+        for (long r = 0; r < G; ++r) {
+            const size_t i = (size_t)c * G + r;
+            const double a = cdt * sigma_of(o, l, r);
+            const double E = std::exp(-a);
+            const double Phi = a > 0 ? -std::expm1(-a) / a : 1.0;
+            o->psi_new[i] = E * (o->psi[i] - cdt * T[i]) + Phi * cdt * ft * q[i];
+        }
+    }
+    o->psi.swap(o->psi_new);
+    o->step_count += 1;
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // C interface for the ctypes wrapper (oracle/rte_oracle.py)
 // ------------------------------------------------------------------------------------------------------------
 // One cell of one step, computed on its own (see orc_step_cell below).
@@ -683,5 +832,32 @@ void orc_streaming(void* h, int formulation, double* T_out) {
 // along the three pencils through the cell.  The _f32 variant reads an fp32 state (values promoted to fp64).
 void orc_step_cell(void* h, const double* psi, int x, int y, int z, double* out) { step_cell_impl<double>(h, psi, x, y, z, out); }
 void orc_step_cell_f32(void* h, const float* psi, int x, int y, int z, double* out) { step_cell_impl<float>(h, psi, x, y, z, out); }
+
+// y = L x  (the steady-state operator above); x, y are [C][G]
+void orc_apply_operator(void* h, int formulation, const double* x, double* y) {
+    Oracle* o = (Oracle*)h;
+    std::vector<double> xv(x, x + o->psi.size()), yv;
+    apply_operator(o, formulation, xv, yv);
+    std::memcpy(y, yv.data(), yv.size() * sizeof(double));
+}
+// q_c(r) = w_c S(r) 1_Omega(r), [C][G]
+void orc_source_field(void* h, double* q) {
+    Oracle* o = (Oracle*)h;
+    std::vector<double> v;
+    source_field(o, v);
+    std::memcpy(q, v.data(), v.size() * sizeof(double));
+}
+// Steady state L psi = q by restarted GMRES(m) from the current state; the state becomes the solution.
+// Returns the number of operator applications.
+long orc_solve_steady(void* h, int formulation, int m, double tol, int max_restarts, double* relres_out) {
+    Oracle* o = (Oracle*)h;
+    std::vector<double> q;
+    source_field(o, q);
+    return gmres_solve(o, formulation, q, o->psi, m, tol, max_restarts, relres_out);
+}
+void orc_step_exp(void* h, int nsteps, int formulation) {
+    Oracle* o = (Oracle*)h;
+    for (int s = 0; s < nsteps; ++s) one_step_exp(o, formulation);
+}
 
 }  // extern "C"

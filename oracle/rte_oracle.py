@@ -49,6 +49,11 @@ def lib():
         L.orc_time_ps.argtypes = [C.c_void_p]
         L.orc_streaming.argtypes = [C.c_void_p, C.c_int, dp]
         L.orc_step_cell.argtypes = [C.c_void_p, dp, C.c_int, C.c_int, C.c_int, dp]
+        L.orc_apply_operator.argtypes = [C.c_void_p, C.c_int, dp, dp]
+        L.orc_source_field.argtypes = [C.c_void_p, dp]
+        L.orc_solve_steady.restype = C.c_long
+        L.orc_solve_steady.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, dp]
+        L.orc_step_exp.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_step_cell_f32.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int, C.c_int, C.c_int, dp]
         _lib = L
     return _lib
@@ -198,6 +203,30 @@ class Oracle:
     def step_ssprk3(self, nsteps=1, formulation=PER_AXIS):
         """NOT the paper's integrator: three-stage SSP Runge-Kutta built from the Euler update."""
         lib().orc_step_ssprk3(self.h, int(nsteps), int(formulation))
+
+    def step_exp(self, nsteps=1, formulation=PER_AXIS):
+        """Exponential (integrating-factor) Euler step, SURVEY §8(f2) / PAPER.md:109 — not eq.(11)."""
+        lib().orc_step_exp(self.h, int(nsteps), int(formulation))
+
+    def apply_operator(self, x, formulation=PER_AXIS):
+        """L x = T[x] + sigma_l x, the steady-state operator of eq.(9)."""
+        x = _f64(x).reshape(self.C, self.nz, self.ny, self.nx)
+        out = np.zeros_like(x)
+        lib().orc_apply_operator(self.h, int(formulation), _dp(x), _dp(out))
+        return out
+
+    def source_field(self):
+        """q_c(r) = w_c S(r) 1_Omega(r) (temporal factor 1)."""
+        out = np.zeros((self.C, self.nz, self.ny, self.nx))
+        lib().orc_source_field(self.h, _dp(out))
+        return out
+
+    def solve_steady(self, restart=30, tol=1e-10, max_restarts=200, formulation=PER_AXIS):
+        """Steady state L psi = q by restarted GMRES from the current state (which becomes the solution).
+        Returns (operator applications, true relative residual)."""
+        rr = C.c_double(0)
+        n = lib().orc_solve_steady(self.h, int(formulation), int(restart), float(tol), int(max_restarts), C.byref(rr))
+        return int(n), float(rr.value)
 
     def time_ps(self):
         return float(lib().orc_time_ps(self.h))

@@ -1,4 +1,4 @@
-"""Pins P1..P12: the fp64 oracle checked against what the paper and the
+"""Pins P1..P16: the fp64 oracle checked against what the paper and the
 mathematics fix, never against itself.  CPU only.
 
 Every expected value below comes from (a) direct quadrature on the sphere / circle written here with numpy + scipy's
@@ -715,3 +715,183 @@ def test_P13_ssprk3_source_stage_times():
     o.step_ssprk3(5)
     got = o.get_state()
     assert np.abs(got[0] - yv).max() < 1e-13 and np.abs(got[1:]).max() < 1e-15
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# P14 — the steady-state operator L = T + sigma_l of eq.(9)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim,N,n,form", [(3, 3, 8, orc.PER_AXIS), (3, 2, 8, orc.LITERAL), (2, 4, 12, orc.PER_AXIS)])
+def test_P14_operator_on_a_single_mode_is_minus_M_over_c(dim, N, n, form):
+    """L Re(v e^{ik.r}) = Re(-(M(k)/c) v e^{ik.r}) with M(k) = -c(i k.A + diag sigma) built from quadrature (P4's)."""
+    rng = np.random.default_rng(14 + dim)
+    dx, c = 0.2, 0.3
+    mu_a, mu_s, g = 0.02, 4.0, 0.8
+    nz = n if dim == 3 else 1
+    j = np.array([1, -2, 3][:dim] + [0] * (3 - dim))
+    kvec = 2 * np.pi * j / (n * dx)
+    C = orc.num_coeffs(dim, N)
+    v = rng.standard_normal(C) + 1j * rng.standard_normal(C)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(n), np.arange(n), indexing="ij")
+    phase = np.exp(1j * dx * (kvec[0] * x + kvec[1] * y + kvec[2] * z))
+    o = orc.Oracle(dim, n, n, nz, N, dx, 1.0, c, mu_a, mu_s, g)
+    got = o.apply_operator((v[:, None, None, None] * phase[None]).real, form)
+    M = mode_matrix(dim, N, kvec, mu_a, mu_s, g, c)
+    ex = (((-M / c) @ v)[:, None, None, None] * phase[None]).real
+    assert np.abs(got - ex).max() < 1e-12 * np.abs(ex).max()
+
+
+def test_P14_operator_diagonal_in_layer_and_omega():
+    """A uniform field has T = 0: L x = sigma_l(r) x cell by cell — mu_b in the layer for every l, mu_a+mu_s(1-g^l) in
+    Omega (hand-written degrees, explicit PML cells: P10's formula)."""
+    n, W, N = 12, 3, 2
+    mu_a, mu_s, g, lo, hi = 0.05, 7.0, 0.8, 0.05, 2.0
+    o = orc.Oracle(3, n, n, n, N, 0.1, 1.0, 0.3, mu_a, mu_s, g, pml_width=W, mu_lo=lo, mu_hi=hi)
+    y = o.apply_operator(np.ones((o.C, n, n, n)))
+    L = hand_degrees(3, N)
+    assert np.allclose(y[:, 6, 6, 6], mu_a + mu_s * (1 - g ** L), rtol=0, atol=1e-14)
+    assert np.allclose(y[:, 6, 6, 0], hi, rtol=0, atol=1e-14)                       # outer face: delta = 1
+    first = lo + (hi - lo) * 0.5 * (1 - math.cos(math.pi / W))                     # first layer cell: delta = 1/W
+    assert np.allclose(y[:, 6, W - 1, 6], first, rtol=0, atol=1e-14)
+    # and the Euler step is psi - c dt (L psi - q): tie the operator to eq.(11) on random data
+    rng = np.random.default_rng(3)
+    psi = rng.standard_normal((o.C, n, n, n))
+    o2 = orc.Oracle(3, n, n, n, N, 0.1, 0.01, 0.3, mu_a, mu_s, g, pml_width=W, mu_lo=lo, mu_hi=hi)
+    o2.set_state(psi)
+    o2.step(1)
+    assert np.abs(o2.get_state() - (psi - 0.3 * 0.01 * o2.apply_operator(psi))).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# P15 — the Krylov steady-state solve (PAPER.md:109): dense solve on a tiny grid, closed form, true residual
+# ------------------------------------------------------------------------------------------------------------------
+def test_P15_gmres_equals_dense_solve_on_a_tiny_grid():
+    n, N = 6, 1
+    rng = np.random.default_rng(15)
+    mu_a = rng.uniform(0.05, 0.5, (n, n, n)); mu_s = rng.uniform(1, 4, (n, n, n)); g = rng.uniform(0.5, 0.9, (n, n, n))
+    o = orc.Oracle(3, n, n, n, N, 0.3, 1.0, 0.3, mu_a, mu_s, g, pml_width=1, mu_lo=0.05, mu_hi=1.5)
+    w = np.array([1.0, 0.2, -0.3, 0.5])
+    S = rng.uniform(0, 1, (2, 2, 2))
+    o.set_source(w, S, (2, 2, 1), (2, 2, 2), 1)
+    q = o.source_field()
+    assert np.count_nonzero(q[0]) == 8 and q[:, 0, :, :].max() == 0          # boxed, nothing in the layer
+    nunk = o.C * n ** 3
+    Lmat = np.zeros((nunk, nunk))
+    e = np.zeros(nunk)
+    for i in range(nunk):                                                     # dense matrix, column by column
+        e[:] = 0; e[i] = 1
+        Lmat[:, i] = o.apply_operator(e.reshape(o.C, n, n, n)).ravel()
+    ex = np.linalg.solve(Lmat, q.ravel()).reshape(q.shape)
+    napp, rr = o.solve_steady(restart=20, tol=1e-12, max_restarts=100)
+    got = o.get_state()
+    assert rr <= 1e-12 and napp > 5
+    assert np.abs(got - ex).max() < 1e-9 * np.abs(ex).max()
+    assert np.linalg.norm(o.apply_operator(got) - q) <= 2e-12 * np.linalg.norm(q)   # its own true residual
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P15_gmres_uniform_source_closed_form(dim):
+    """Uniform constant source in a uniform periodic medium: psi_c = q_c / sigma_l (P7's closed form)."""
+    n = 6
+    nz = n if dim == 3 else 1
+    mu_a, mu_s, g = 0.5, 3.0, 0.5
+    o = orc.Oracle(dim, n, n, nz, 2, 0.1, 1.0, 0.3, mu_a, mu_s, g)
+    w = np.arange(1, o.C + 1) * 0.25
+    o.set_source(w, np.full((nz, n, n), 2.0), (0, 0, 0), (n, n, nz), 1)
+    o.solve_steady(restart=10, tol=1e-13, max_restarts=20)
+    L = hand_degrees(dim, 2)
+    fixed = 2.0 * w / (mu_a + mu_s * (1 - g ** L))
+    assert np.abs(o.get_state() - fixed[:, None, None, None]).max() < 1e-11 * fixed.max()
+
+
+def test_P15_steady_state_is_the_fixed_point_of_the_paper_step():
+    """The GMRES solution does not move under the paper's Euler step eq.(11) with the same constant source."""
+    n, N = 8, 2
+    rng = np.random.default_rng(16)
+    mu_s = rng.uniform(2, 6, (n, n, n))
+    o = orc.Oracle(3, n, n, n, N, 0.25, 0.01, 0.3, 0.1, mu_s, 0.7, pml_width=2, mu_lo=0.1, mu_hi=2.0)
+    w = np.zeros(o.C); w[0] = 1.0; w[2] = 0.5
+    o.set_source(w, np.ones((1, 2, 2)), (3, 3, 3), (2, 2, 1), 1)
+    o.solve_steady(restart=30, tol=1e-12, max_restarts=200)
+    ss = o.get_state()
+    o.step(5)
+    assert np.abs(o.get_state() - ss).max() < 1e-11 * np.abs(ss).max()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# P16 — exponential (integrating-factor) Euler step (SURVEY §8(f2), PAPER.md:109): exact diagonal, exact source response
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim,form", [(3, orc.PER_AXIS), (2, orc.LITERAL)])
+def test_P16_exp_step_uniform_decay_is_exact(dim, form):
+    n, N = 6, 3
+    nz = n if dim == 3 else 1
+    mu_a, mu_s, g, c, dt = 0.013, 9.0, 0.87, 0.3, 0.35            # c dt sigma_l up to ~0.4: Euler would be far off
+    o = orc.Oracle(dim, n, n, nz, N, 0.1, dt, c, mu_a, mu_s, g)
+    amp = 1.0 + np.arange(o.C)
+    o.set_state(np.broadcast_to(amp[:, None, None, None], (o.C, nz, n, n)))
+    o.step_exp(11, form)
+    L = hand_degrees(dim, N)
+    ex = amp * np.exp(-c * (mu_a + mu_s * (1 - g ** L)) * 11 * dt)
+    # (round-off of the spectral derivative of a constant, ~1e-14 k_max, enters times c dt = 0.1 per step)
+    assert np.abs(o.get_state() - ex[:, None, None, None]).max() < 1e-11 * amp.max()
+    assert abs(o.time_ps() - 11 * dt) < 1e-15
+
+
+def test_P16_exp_step_exact_in_layer_and_source_response():
+    """Whole-domain layer: every l decays as exp(-c mu_b t) exactly.  Uniform constant source from zero:
+    psi_c(t_n) = (q_c/sigma_l)(1 - exp(-c sigma_l t_n)) exactly (phi_1 weighting), fixed point q_c/sigma_l."""
+    n, c, dt = 8, 0.3, 0.5
+    o = orc.Oracle(3, n, n, n, 2, 0.1, dt, c, 0.01, 10.0, 0.9, pml_width=4, mu_lo=0.7, mu_hi=0.7)
+    amp = 1.0 + np.arange(o.C)
+    o.set_state(np.broadcast_to(amp[:, None, None, None], (o.C, n, n, n)))
+    o.step_exp(6)
+    assert np.abs(o.get_state() - (amp * math.exp(-c * 0.7 * 6 * dt))[:, None, None, None]).max() < 1e-11 * amp.max()
+    mu_a, mu_s, g = 0.5, 3.0, 0.5
+    o2 = orc.Oracle(3, 4, 4, 4, 2, 0.1, dt, c, mu_a, mu_s, g)
+    w = np.arange(1, o2.C + 1) * 0.25
+    o2.set_source(w, np.full((4, 4, 4), 2.0), (0, 0, 0), (4, 4, 4), 1)
+    o2.step_exp(9)
+    sigma = mu_a + mu_s * (1 - g ** hand_degrees(3, 2))
+    ex = 2.0 * w / sigma * (1 - np.exp(-c * sigma * 9 * dt))
+    assert np.abs(o2.get_state() - ex[:, None, None, None]).max() < 1e-11 * ex.max()
+
+
+def test_P16_exp_step_single_mode_matrix_and_convergence():
+    """One Fourier mode: psi_{n+1} = diag(E) (I - c dt i k.A) psi_n with E = exp(-c dt sigma_l), A from quadrature;
+    first-order convergence to expm(M t); and the diagonal no longer limits dt: with streaming switched off by k = 0
+    the step is exact at c dt sigma = 6 where eq.(11) blows up."""
+    from scipy.linalg import expm
+    dim, N, n = 3, 3, 8
+    dx, c, dt = 0.2, 0.3, 0.002
+    mu_a, mu_s, g = 0.02, 4.0, 0.8
+    kvec = 2 * np.pi * np.array([2, -1, 3]) / (n * dx)
+    C = orc.num_coeffs(dim, N)
+    rng = np.random.default_rng(160)
+    v = rng.standard_normal(C) + 1j * rng.standard_normal(C)
+    z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    phase = np.exp(1j * dx * (kvec[0] * x + kvec[1] * y + kvec[2] * z))
+    A = quad_coupling(dim, N)
+    sigma = mu_a + mu_s * (1 - g ** hand_degrees(dim, N))
+    kA = sum(kvec[a] * A[a] for a in range(dim))
+    step = np.diag(np.exp(-c * dt * sigma)) @ (np.eye(C) - c * dt * 1j * kA)
+    o = orc.Oracle(dim, n, n, n, N, dx, dt, c, mu_a, mu_s, g)
+    o.set_state((v[:, None, None, None] * phase[None]).real)
+    o.step_exp(20)
+    ex = ((np.linalg.matrix_power(step, 20) @ v)[:, None, None, None] * phase[None]).real
+    assert np.abs(o.get_state() - ex).max() < 1e-12 * np.abs(v).max()
+    M = mode_matrix(dim, N, kvec, mu_a, mu_s, g, c)
+    t, errs = 0.04, []
+    for steps in (20, 40):
+        o = orc.Oracle(dim, n, n, n, N, dx, t / steps, c, mu_a, mu_s, g)
+        o.set_state((v[:, None, None, None] * phase[None]).real)
+        o.step_exp(steps)
+        errs.append(np.abs(o.get_state() - ((expm(M * t) @ v)[:, None, None, None] * phase[None]).real).max())
+    assert 1.7 < errs[0] / errs[1] < 2.3
+    # stiff diagonal: c dt sigma_1 = 0.3 * 20 * 1.0 = 6
+    big = orc.Oracle(dim, n, n, n, 1, dx, 20.0, c, 0.5, 1.0, 0.5)
+    big.set_state(np.ones((4, n, n, n)))
+    big.step_exp(3)
+    assert np.allclose(big.get_state()[1], math.exp(-c * 1.0 * 60.0), rtol=1e-12, atol=0)
+    eul = orc.Oracle(dim, n, n, n, 1, dx, 20.0, c, 0.5, 1.0, 0.5)
+    eul.set_state(np.ones((4, n, n, n)))
+    eul.step(3)
+    assert abs(eul.get_state()[1, 0, 0, 0]) > 100          # (1 - 6)^3 = -125
