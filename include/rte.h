@@ -17,7 +17,11 @@
  * Conventions
  *   units            mm, ps, mm^-1 (as the paper)
  *   grid             nx*ny*nz cells, x fastest; cell i along an axis sits at (i - n/2) dx; nz = 1 when dim = 2.
- *                    Every extent must be one of 16,32,48,64,96,128,192,256,384,512.
+ *                    Every extent must be an EVEN number of the form 2^a 3^b in [16, 1024] (16, 18, 24, 32, 36, 48, 54,
+ *                    64, 72, 96, 108, 128, 144, 162, 192, 216, 256, 288, 324, 384, 432, 486, 512, 576, 648, 768, 864,
+ *                    972, 1024), and one pencil of all coefficients must fit a shared-memory tile
+ *                    (n * 8 * ceil(C/2) bytes + the diagonal table <= 226 KB; else RTE_EUNSUPPORTED).
+ *   order            1 <= N <= 31 (at most 1024 coefficients in 3-D); larger N is RTE_EINVAL / a negative count.
  *   coefficients     3-D: C=(N+1)^2, c = l*l + l + m; m>=0 is the cos-type real harmonic a_l^m, m<0 the sin-type
  *                    b_l^|m| (R6).  2-D: C=2N+1, c=0 -> a_0, c=2m-1 -> a_m, c=2m -> b_m (R8).
  *                    Coefficient 0 is the fluence in both (R9).
@@ -89,14 +93,29 @@ int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* 
  * accumulates the next state into the other, then they trade places — and three per-cell coefficient maps). */
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out);
 
+/* Bytes of n_fields additional state-sized device buffers (caller-owned, handed over with rte_set_extra_workspace):
+ * rte_step_ssprk3 needs 1 field, rte_apply_operator 2, rte_solve_steady restart + 3. */
+int rte_extra_workspace_bytes(const rte_grid* grid, int N, int n_fields, size_t* bytes_out);
+
+/* Forward-Euler stability bound of the step eq.(11) (R10; the paper picks dt "by inspection", PAPER.md:141,
+ * "time-steps of the order of 100 fs provide stability").  Forward Euler is stabilised only by the
+ * scattering damping: for every Fourier mode the eigenvalues lambda of M(k) = -c (i k A + diag sigma_l),
+ * sigma_l = mu_a + mu_s (1 - g^l), must satisfy dt <= -2 Re(lambda) / |lambda|^2.  The bound is evaluated on 200
+ * wavenumber magnitudes up to the corner Nyquist sqrt(dim) (pi/dx)(1 - 2/n_min) (k along one axis: rotational
+ * invariance) for ONE medium — pass the weakest damping present: smallest mu_a and mu_s, largest g.
+ * bound_ps_out: the bound; dt_ps_out: the recommended step, half of it (a PML moves the true bound by x0.7-2).
+ * Either output may be NULL.  Host only. */
+int rte_stable_dt(int dim, int N, int n_min, float dx_mm, float c_mm_per_ps, float mu_a_min, float mu_s_min,
+                  float g_max, double* bound_ps_out, double* dt_ps_out);
+
 /* ---- life cycle ---------------------------------------------------------------------------------------------- */
 
 /* Build a solver: validates, generates the coupling tables, wavenumbers (k at Nyquist = 0, R5), FFT
  * twiddles and the per-cell sigma / PML maps on the device, zeroes the state, sets t = 0.
  * workspace_dev: caller-owned device memory of at least rte_workspace_bytes, 256-byte aligned, alive until
  * rte_destroy.  cuda_stream: a cudaStream_t (may be NULL).
- * RTE_EINVAL: N<1, dx/dt/c <= 0, unsupported extent, dim/grid mismatch, PML too wide, workspace too small or
- * misaligned.  RTE_ECUDA: no sm_100 device or a CUDA failure.  The time step is NOT checked for stability
+ * RTE_EINVAL: N<1 or N>31, dx/dt/c <= 0, unsupported extent, dim/grid mismatch, PML too wide, workspace too small or
+ * misaligned.  RTE_EUNSUPPORTED: a pencil of all coefficients does not fit one shared-memory tile.  RTE_ECUDA: no sm_100 device or a CUDA failure.  The time step is NOT checked for stability
  * (the paper chooses dt "by inspection"). */
 int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx_mm, float dt_ps, float c_mm_per_ps,
                const rte_media* media, const rte_pml* pml, void* workspace_dev, size_t workspace_bytes,
@@ -128,8 +147,40 @@ int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, 
 /* Advance nsteps forward-Euler steps (eq.(11)); asynchronous on the stream.  One step = one pencil-FFT
  * kernel per axis (coupling -> DFT -> i k -> IDFT, eq.(6)-(10)): the x kernel also applies scattering, PML and source
  * (eq.(9),(12)) and stores psi(1 - c dt sigma_l) + c dt q - c dt T_x into the second state buffer, the other axes add
- * their -c dt T_a to it; the buffers then trade places.  Results are bit-reproducible from run to run. */
+ * their -c dt T_a to it; the buffers then trade places.  Results are bit-reproducible from run to run.
+ * Grids whose state is at most 24 MB (L2-resident, launch-bound) replay the same launches from a CUDA graph, 32 steps
+ * per replay; the results are identical to the eager path. */
 int rte_step(rte_ctx* ctx, int nsteps);
+
+/* Hand the library additional caller-owned device memory (256-byte aligned; rte_extra_workspace_bytes) that it keeps
+ * until rte_destroy or the next call of this function (extra_dev = NULL takes it back).  Synchronises the stream. */
+int rte_set_extra_workspace(rte_ctx* ctx, void* extra_dev, size_t bytes);
+
+/* NOT eq.(11): nsteps steps of the exponential (integrating-factor) Euler scheme, the family PAPER.md:109 and :195
+ * point to ("exponential integrators").  The diagonal part of eq.(9) is integrated exactly, the
+ * streaming term explicitly, the source through phi_1:
+ *     psi^{n+1} = E (psi^n - c dt T[psi^n]) + Phi c dt q(t_n),   E = exp(-c dt sigma_l),  Phi = (1 - E)/(c dt sigma_l).
+ * A uniform field decays as exp(-c sigma_l t) with no O(dt) error, also in the PML, and the stiff diagonal
+ * (c dt sigma_l > 2, where eq.(11) diverges) no longer bounds dt; the streaming bound (rte_stable_dt) is unchanged to
+ * leading order.  Runs on the generic kernels.  Asynchronous on the stream. */
+int rte_step_exp(rte_ctx* ctx, int nsteps);
+
+/* The time-independent transport operator of eq.(9): y = L x = T[x] + sigma_l x, so that eq.(9) reads
+ * d psi/dt = -c L psi + c q and a steady state satisfies L psi = q ("repeated application of the implicit operator",
+ * PAPER.md:109).  x_dev, y_dev: [C][nz][ny][nx] fp32 device arrays.  The state and the clock are untouched.
+ * Needs 2 fields of extra workspace.  Asynchronous on the stream. */
+int rte_apply_operator(rte_ctx* ctx, const float* x_dev, float* y_dev);
+
+/* Steady state L psi = q (q = the source of rte_set_source with temporal factor 1) by restarted GMRES(restart),
+ * entirely on the device (the paper's Krylov solver was bound by host<->device
+ * transfers).  The current state is the initial guess and becomes the solution.  Stops when the true relative
+ * residual ||q - L psi|| / ||q||, recomputed at every restart, is <= tol, or after max_restarts cycles (not an
+ * error: check *relres_out).  The Krylov basis, the Hessenberg matrix and the rotations live in device memory;
+ * dot products / updates are this library's kernels; the host reads a few scalars once per restart cycle.
+ * Needs restart + 3 fields of extra workspace; 1 <= restart <= 64.  applications_out: operator applications done;
+ * relres_out: final true relative residual (either may be NULL).  Synchronises the stream. */
+int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int* applications_out,
+                     double* relres_out);
 
 /* NOT the paper's integrator (the paper uses forward Euler and names better integrators as future work,
  * PAPER.md:109,195): nsteps steps of the three-stage, third-order strong-stability-preserving Runge-Kutta scheme
@@ -137,7 +188,7 @@ int rte_step(rte_ctx* ctx, int nsteps);
  *   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2).
  * Its stability region contains the imaginary axis up to sqrt(3), so dt may approach dx/c instead of the
  * scattering-limited Euler bound (R10).  Three Euler updates (9 pass kernels in 3-D) and two state-wide
- * axpby kernels per step; allocates one extra state buffer (library-owned) on first use: RTE_ENOMEM if that fails.
+ * axpby kernels per step.  Needs 1 field of extra workspace (rte_set_extra_workspace), RTE_EINVAL without it.
  * Asynchronous on the stream; rte_time_ps advances by dt per step. */
 int rte_step_ssprk3(rte_ctx* ctx, int nsteps);
 

@@ -564,7 +564,9 @@ static long gmres_solve(Oracle* o, int formulation, const std::vector<double>& b
             for (int j = 0; j <= k; ++j) {                       // modified Gram-Schmidt
                 const double h = dot(w, V[j]);
                 H[(size_t)j * m + k] = h;
-                for (size_t i = 0; i < n; ++i) w[i] -= h * V[j][i];
+                const double* vj = V[j].data();
+#pragma omp parallel for schedule(static)
+                for (long i = 0; i < (long)n; ++i) w[i] -= h * vj[i];
             }
             const double hn = std::sqrt(dot(w, w));
             H[(size_t)(k + 1) * m + k] = hn;
@@ -590,8 +592,11 @@ static long gmres_solve(Oracle* o, int formulation, const std::vector<double>& b
             for (int j = i + 1; j < k; ++j) s -= H[(size_t)i * m + j] * yv[j];
             yv[i] = s / H[(size_t)i * m + i];
         }
-        for (int j = 0; j < k; ++j)
-            for (size_t i = 0; i < n; ++i) x[i] += yv[j] * V[j][i];
+        for (int j = 0; j < k; ++j) {
+            const double* vj = V[j].data();
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < (long)n; ++i) x[i] += yv[j] * vj[i];
+        }
     }
     *relres_out = relres;
     return applications;

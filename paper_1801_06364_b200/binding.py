@@ -58,6 +58,12 @@ _lib.rte_set_source.argtypes = [_vp, C.POINTER(C.c_float), _vp, _i3, _i3, _i, _f
 _lib.rte_set_source_host.argtypes = [_vp, C.POINTER(C.c_float), _vp, _i3, _i3, _i, _f, _f]
 _lib.rte_step.argtypes = [_vp, _i]
 _lib.rte_step_ssprk3.argtypes = [_vp, _i]
+_lib.rte_step_exp.argtypes = [_vp, _i]
+_lib.rte_extra_workspace_bytes.argtypes = [C.POINTER(rte_grid), _i, _i, C.POINTER(C.c_size_t)]
+_lib.rte_set_extra_workspace.argtypes = [_vp, _vp, C.c_size_t]
+_lib.rte_stable_dt.argtypes = [_i, _i, _i, _f, _f, _f, _f, _f, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+_lib.rte_apply_operator.argtypes = [_vp, _vp, _vp]
+_lib.rte_solve_steady.argtypes = [_vp, _i, C.c_double, _i, C.POINTER(_i), C.POINTER(C.c_double)]
 _lib.rte_step_profile.argtypes = [_vp, _i, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
 _lib.rte_fluence_change.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rte_time_ps.argtypes = [_vp, C.POINTER(C.c_double)]
@@ -72,7 +78,9 @@ _lib.rte_pml_profile.argtypes = [C.POINTER(rte_grid), C.POINTER(rte_pml), _vp, _
 
 EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_workspace_bytes", "rte_create", "rte_destroy",
             "rte_set_state", "rte_get_state", "rte_set_state_host", "rte_get_state_host", "rte_reset_time",
-            "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_ssprk3", "rte_step_profile", "rte_fluence", "rte_fluence_host",
+            "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_ssprk3", "rte_step_exp", "rte_step_profile",
+            "rte_extra_workspace_bytes", "rte_set_extra_workspace", "rte_stable_dt", "rte_apply_operator",
+            "rte_solve_steady", "rte_fluence", "rte_fluence_host",
             "rte_fluence_change", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
             "rte_media_ellipsoids", "rte_media_lognormal", "rte_pml_profile"]
 
@@ -241,9 +249,63 @@ def rte_step(ctx, nsteps=1):
     _check(_lib.rte_step(ctx.handle, int(nsteps)), ctx.handle)
 
 
+def rte_extra_workspace_bytes(grid, N, n_fields):
+    out = C.c_size_t(0)
+    g = _grid(grid)
+    _check(_lib.rte_extra_workspace_bytes(C.byref(g), N, int(n_fields), C.byref(out)))
+    return int(out.value)
+
+
+def rte_set_extra_workspace(ctx, n_fields):
+    """Allocate n_fields state-sized device buffers with torch (the caller-owned extra workspace of include/rte.h),
+    hand them to the library and keep them alive with the context.  n_fields = 0 takes the workspace back."""
+    if n_fields <= 0:
+        _check(_lib.rte_set_extra_workspace(ctx.handle, None, 0), ctx.handle)
+        ctx._extra, ctx._extra_fields = None, 0
+        return
+    if getattr(ctx, "_extra_fields", 0) >= n_fields:
+        return
+    nbytes = rte_extra_workspace_bytes(ctx.grid, ctx.N, n_fields)
+    _check(_lib.rte_set_extra_workspace(ctx.handle, None, 0), ctx.handle)     # drop (and free) the old one first
+    ctx._extra = None
+    buf = torch.empty(nbytes, dtype=torch.uint8, device=ctx.device)
+    _check(_lib.rte_set_extra_workspace(ctx.handle, C.c_void_p(buf.data_ptr()), nbytes), ctx.handle)
+    ctx._extra, ctx._extra_fields = buf, n_fields
+
+
+def rte_stable_dt(dim, N, n_min, dx_mm, c_mm_per_ps, mu_a_min, mu_s_min, g_max):
+    """(bound, recommended dt = bound / 2) of the forward-Euler step in ps (host only; include/rte.h)."""
+    b, d = C.c_double(0), C.c_double(0)
+    _check(_lib.rte_stable_dt(int(dim), int(N), int(n_min), float(dx_mm), float(c_mm_per_ps), float(mu_a_min),
+                              float(mu_s_min), float(g_max), C.byref(b), C.byref(d)))
+    return float(b.value), float(d.value)
+
+
 def rte_step_ssprk3(ctx, nsteps=1):
     """NOT the paper's integrator: SSP-RK3 built from the Euler update (include/rte.h)."""
+    rte_set_extra_workspace(ctx, max(1, getattr(ctx, "_extra_fields", 0)))
     _check(_lib.rte_step_ssprk3(ctx.handle, int(nsteps)), ctx.handle)
+
+
+def rte_step_exp(ctx, nsteps=1):
+    """Exponential (integrating-factor) Euler step (include/rte.h) — not eq.(11)."""
+    _check(_lib.rte_step_exp(ctx.handle, int(nsteps)), ctx.handle)
+
+
+def rte_apply_operator(ctx, x_dev, y_dev):
+    """y = L x = T[x] + sigma_l x (include/rte.h); [C,nz,ny,nx] fp32 CUDA tensors."""
+    rte_set_extra_workspace(ctx, max(2, getattr(ctx, "_extra_fields", 0)))
+    _check(_lib.rte_apply_operator(ctx.handle, _dev(x_dev), _dev(y_dev)), ctx.handle)
+
+
+def rte_solve_steady(ctx, restart=30, tol=1e-5, max_restarts=100):
+    """Device-resident GMRES(restart) for L psi = q from the current state; returns (operator applications,
+    true relative residual).  Allocates restart + 3 fields of extra workspace if the context has fewer."""
+    rte_set_extra_workspace(ctx, max(restart + 3, getattr(ctx, "_extra_fields", 0)))
+    n, rr = _i(0), C.c_double(0)
+    _check(_lib.rte_solve_steady(ctx.handle, int(restart), float(tol), int(max_restarts), C.byref(n), C.byref(rr)),
+           ctx.handle)
+    return int(n.value), float(rr.value)
 
 
 def rte_step_profile(ctx, nsteps=1):

@@ -7,15 +7,18 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <string>
 #include <utility>
 #include <vector>
 
 #include "rte_pass.cuh"
+#include "rte_solver.cuh"
 #include "rte_tables.h"
 
 using rtepass::CplEntry;
@@ -26,8 +29,17 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct AxisTables {
-    CplEntry* cpl = nullptr;
+    CplEntry* cpl = nullptr;      // weights x (-c dt) (2 pi / (n dx)) / n : the time step (eq.(11))
+    CplEntry* cpl_op = nullptr;   // weights x (+1)    (2 pi / (n dx)) / n : the steady-state operator L = T + sigma_l
+    float2* tw = nullptr;         // forward twiddles of this axis (generic kernels)
     int n = 0, N1 = 0, N2 = 0, maxcnt = 0, npure = 0;   // npure: leading coupling slots with pure blocks (rte_tables.h)
+};
+
+// what a sweep of the three pass kernels computes
+enum PassKind {
+    KIND_STEP = 0,   // out = in (1 - c dt sigma_l) - c dt T[in] + c dt q            eq.(11)
+    KIND_OPER = 1,   // out = sigma_l in + T[in]                                     L of eq.(9)
+    KIND_EXP = 2     // out = E (in - c dt T[in]) + phi_1 c dt q, E = exp(-c dt sigma_l)   exponential Euler
 };
 
 }  // namespace
@@ -51,7 +63,13 @@ struct rte_ctx {
     float* srcS = nullptr;
     size_t srcS_cap = 0;
     float g_uniform = 0.f;         // > 0: the anisotropy g is one number (media.g_is_map == 0): kernels use the 2-number table
-    float2* extra = nullptr;       // third state buffer, library-owned, allocated by the first rte_step_ssprk3
+    char* extra = nullptr;         // caller-owned extra workspace (rte_set_extra_workspace): state-sized fields for
+    size_t extra_bytes = 0;        // rte_step_ssprk3 (1), rte_apply_operator (2), rte_solve_steady (restart + 3)
+    rtesolve::Scalars* sc = nullptr;   // device scalars of the Krylov solver
+    double* partial = nullptr;         // per-block partial sums of its reductions
+    cudaGraphExec_t graph = nullptr;   // rte_step_graph: two captured steps (the state buffers are back in place)
+    bool graph_has_source = false;
+    float* graph_amp = nullptr;        // device table of c dt f(t_n) for the captured steps
     float* phi_prev = nullptr;
     double* red = nullptr;         // 2 doubles for reductions
     bool have_prev = false;
@@ -61,6 +79,7 @@ struct rte_ctx {
     double src_t0 = 0, src_sig = 1;
     long long steps = 0;
     long long launches = 0;
+    int launches_warm = 0;         // an eager step has run (kernel attributes set): graph capture is safe
     char err[256] = "";
 };
 
@@ -71,6 +90,16 @@ int fail(rte_ctx* ctx, int code, const char* fmt, const char* detail = "") {
     snprintf(dst, 256, fmt, detail);
     return code;
 }
+
+// nothing throws across the ABI: std::bad_alloc -> RTE_ENOMEM, anything else -> RTE_EINVAL
+template <typename F>
+int guarded(F&& f) {
+    try { return f(); }
+    catch (const std::bad_alloc&) { return RTE_ENOMEM; }
+    catch (...) { return RTE_EINVAL; }
+}
+
+constexpr int kMaxOrder = 31;   // P_N orders the tables are built for (N = 31: 1024 coefficients in 3-D)
 
 #define CUDA_TRY(ctx, expr)                                                              \
     do {                                                                                 \
@@ -215,7 +244,7 @@ __global__ void k_source_copy(float* __restrict__ dst, const float* __restrict__
 
 // sum over Omega of (phi - prev)^2 and phi^2 ; then prev <- phi
 __global__ void k_fluence_change(const float* __restrict__ psi, float* __restrict__ prev, double* __restrict__ red,
-                                 const float* __restrict__ ss_unused, int dim, int nx, int ny, int nz, int W, int Cp) {
+                                 int dim, int nx, int ny, int nz, int W, int Cp) {
     const long long G = (long long)nx * ny * nz;
     double d2 = 0, n2 = 0;
     for (long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x; cell < G;
@@ -350,7 +379,7 @@ int check_grid(const rte_grid* g) {
 // pass dispatch
 // ---------------------------------------------------------------------------------------------------------------------
 // A pass runs either a kernel specialised at compile time for (n, P, TP, block size) — the five BASELINE.json
-// configurations — or the generic kernel (run-time P, TP, block size) for every other supported extent / order.
+// configurations — or the generic kernel (run-time P, TP, block size, FIRST/ACC) for every other supported extent / order.
 struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; };
 
 struct SpecRow { int n, P, TP, nt; };
@@ -371,7 +400,7 @@ size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
 
 constexpr size_t kMaxSmem = 226 * 1024;   // 227 KB per CTA minus the static mbarrier slot
 
-LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
+LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz;
     int groups = 1;
     if (axis == 0) { A.stride_i = 1; A.stride_t = nx; A.group_stride = 0; A.pencils_per_group = ny * nz; }
@@ -380,16 +409,18 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
     } else { A.stride_i = nx * ny; A.stride_t = 1; A.group_stride = 0; A.pencils_per_group = nx * ny; }
     const AxisTables& T = c->ax[axis];
     const int P = c->P, n = T.n;
-    const bool first = axis == 0, diag = first;   // the x pass carries the Euler diagonal table
+    const bool first = axis == 0;
+    const bool diag = first || kind == KIND_EXP;   // the x pass carries the Euler diagonal table (every pass of the exponential step)
     LaunchPlan L{};
     L.spec = -1;
     A.P = P;
-    for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
-        if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
-            !(axis == 2 && T.maxcnt > 2) && !(axis < 2 && T.npure < 2)) {
-            L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
-            break;
-        }
+    if (kind != KIND_EXP)                          // the exponential step runs on the generic kernels
+        for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
+            if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
+                !(axis == 2 && T.maxcnt > 2) && !(axis < 2 && T.npure < 2)) {
+                L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
+                break;
+            }
     if (L.spec < 0) {
         int tp = 1;
         while (tp * P < 32 && tp < 8) tp *= 2;
@@ -398,7 +429,8 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A) {
         const int Q = tp * P;
         const int T1 = Q * T.N2, T2 = Q * T.N1;
         int best = 128; double best_cost = 1e30;
-        for (int nt = 64; nt <= 320; nt += 32) {
+        const int ntmax = T.N1 > 32 ? 224 : 320;   // 36-point register transforms: 255 registers x 224 threads fit one SM
+        for (int nt = 64; nt <= ntmax; nt += 32) {
             if (nt > T1 && nt > T2 && nt > 64) break;
             const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;
             const double cost = w1 + w2;
@@ -418,14 +450,18 @@ template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bo
 cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG>;
     // the dynamic shared-memory limit is a per-device function attribute: set it once per (kernel instance, device)
+    static std::mutex mu;
     static bool configured[64] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64 || !configured[dev]) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) configured[dev] = true;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (dev < 0 || dev >= 64 || !configured[dev]) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+            if (e != cudaSuccess) return e;
+            if (dev >= 0 && dev < 64) configured[dev] = true;
+        }
     }
     kern<<<L.blocks, L.nt, L.smem, s>>>(A);
     return cudaGetLastError();
@@ -437,38 +473,31 @@ cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
 cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     constexpr bool kHasUG = MODE == rtepass::MODE_FIRST && QC != 0 && (QC / (PC ? PC : 1)) > 1;
-    if (kHasUG && A.g_uniform > 0.f) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, kHasUG>(A, L, s);
+    if constexpr (kHasUG)
+        if (A.g_uniform > 0.f) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, true>(A, L, s);
     PassArgs B = A;
     B.g_uniform = 0.f;                 // every other instance builds and reads the N+1-number table
     return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, false>(B, L, s);
 }
 
-template <int MODE>
+// generic kernels: one instance per supported pencil length (rte_tables.h RTE_SPLITS), FIRST/ACC at run time
 cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
-    switch (n) {
-        case 16: return launch_one<4, 4, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 32: return launch_one<4, 8, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 48: return launch_one<4, 12, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 64: return launch_one<8, 8, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 96: return launch_one<8, 12, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 128: return launch_one<8, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 192: return launch_one<12, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 256: return launch_one<16, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 384: return launch_one<24, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        case 512: return launch_one<32, 16, MODE, 4, 0, 0, 0, 1>(A, L, s);
-        default: return cudaErrorInvalidValue;
-    }
+#define RTE_GENERIC_CASE(N1_, N2_) \
+    if (n == (N1_) * (N2_)) return launch_one<N1_, N2_, rtepass::MODE_RT, 4, 0, 0, 0, 1>(A, L, s);
+    RTE_SPLITS(RTE_GENERIC_CASE)
+#undef RTE_GENERIC_CASE
+    return cudaErrorInvalidValue;
 }
 
-// E = 2 on the z axis of 3-D runs (fan-in of the z coupling is at most 2 pairs, rte_tables.h), 4 otherwise
+// E = 2 on the z axis of 3-D runs (fan-in of the z coupling is at most 2 pairs, rte_tables.h), 4 otherwise.
+// FIRST and ACC instances differ in occupancy (the accumulating tails hold no loaded data): MINB per mode.
 template <int MODE, int E>
 cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
+    constexpr bool F = MODE == rtepass::MODE_FIRST;
     switch (spec) {
         case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2>(A, L, s);
-        case 1: return MODE == rtepass::MODE_FIRST ? launch_one<16, 16, MODE, E, 36, 18, 288, 2>(A, L, s)
-                                                   : launch_one<16, 16, MODE, E, 36, 18, 288, 3>(A, L, s);
-        case 2: return MODE == rtepass::MODE_FIRST ? launch_one<16, 8, MODE, E, 32, 8, 256, 3>(A, L, s)
-                                                   : launch_one<16, 8, MODE, E, 32, 8, 256, 4>(A, L, s);
+        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3>(A, L, s);
+        case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, F ? 3 : 4>(A, L, s);
         case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2>(A, L, s);
         case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3>(A, L, s);
         case 5: return launch_one<8, 8, MODE, E, 32, 32, 256, 3>(A, L, s);
@@ -482,34 +511,43 @@ double source_time_factor(const rte_ctx* c, double t) {
     return 0.0;
 }
 
-// One forward-Euler update of eq.(11): out = in - c dt ( T[in] + sigma_l in ) + c dt q(t_src) — one pass kernel per axis.
-int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, cudaEvent_t* ev = nullptr) {
+// One sweep of the per-axis pass kernels, out = F(in) with F chosen by `kind` (PassKind above): the forward-Euler update
+// of eq.(11) with the source at t_src, the steady-state operator, or the exponential Euler update.
+// amp_dev (optional): device location of c dt f(t) for this sweep (CUDA-graph replay), instead of the host value.
+int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKind kind = KIND_STEP,
+                 cudaEvent_t* ev = nullptr, const int* halt = nullptr, const float* amp_dev = nullptr) {
     const int naxes = c->grid.dim;
     for (int axis = 0; axis < naxes; ++axis) {
         PassArgs A{};
         A.psi = in; A.acc = out;
-        A.cpl = c->ax[axis].cpl;
+        A.cpl = kind == KIND_OPER ? c->ax[axis].cpl_op : c->ax[axis].cpl;
+        A.tw = c->ax[axis].tw;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
-        A.cdt = c->c * c->dt; A.nsig = c->N + 1; A.g_uniform = c->g_uniform;
+        A.cdt = kind == KIND_OPER ? -1.f : c->c * c->dt;
+        A.ident = kind == KIND_OPER ? 0.f : 1.f;
+        A.expo = kind == KIND_EXP ? 1 : 0;
+        A.first = axis == 0 ? 1 : 0;
+        A.halt = halt;
+        A.nsig = c->N + 1; A.g_uniform = c->g_uniform;
         A.srcS = c->srcS; A.srcw = c->srcw;
         for (int k = 0; k < 3; ++k) { A.src_org[k] = c->src_org[k]; A.src_ext[k] = c->src_ext[k]; }
-        A.src_amp = 0.f;
+        A.src_amp = 0.f; A.src_amp_dev = nullptr;
         A.nx = c->grid.nx; A.ny = c->grid.ny;
-        const LaunchPlan L = plan_pass(c, axis, A);
+        const LaunchPlan L = plan_pass(c, axis, A, kind);
         const int n = c->ax[axis].n;
         cudaError_t e;
         if (axis == 0) {
-            if (c->src_kind != 0)
+            if (c->src_kind != 0 && kind != KIND_OPER) {
                 A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src));
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream)
-                            : launch_generic<rtepass::MODE_FIRST>(n, A, L, c->stream);
+                A.src_amp_dev = amp_dev;
+                if (amp_dev) A.src_amp = 1.f;      // non-zero: the kernel reads the device value
+            }
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
         } else if (axis == 2) {
             // z axis: coupling fan-in 2 (rte_tables.h); plan_pass falls back to the generic kernel otherwise
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 2>(L.spec, A, L, c->stream)
-                            : launch_generic<rtepass::MODE_ACC>(n, A, L, c->stream);
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 2>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
         } else {
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 4>(L.spec, A, L, c->stream)
-                            : launch_generic<rtepass::MODE_ACC>(n, A, L, c->stream);
+            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 4>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
         }
         if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
         c->launches += 1;
@@ -519,8 +557,8 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, cudaEv
 }
 
 // the paper's step: psi^{n+1} = Euler update of psi^n with the source at t_n (R14); the two state buffers trade places
-int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr) {
-    const int rc = euler_update(c, c->psi, c->part, (double)c->steps * (double)c->dt, ev);
+int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr, PassKind kind = KIND_STEP, const float* amp_dev = nullptr) {
+    const int rc = euler_update(c, c->psi, c->part, (double)c->steps * (double)c->dt, kind, ev, nullptr, amp_dev);
     if (rc != RTE_OK) return rc;
     std::swap(c->psi, c->part);
     c->steps += 1;
@@ -538,17 +576,21 @@ __global__ void k_axpby(float4* __restrict__ y, const float4* __restrict__ x, fl
     }
 }
 
+size_t field_bytes(const rte_ctx* c) { return align_up((size_t)c->G * c->Cp * sizeof(float), 256); }
+
+// i-th state-sized field of the caller's extra workspace, or nullptr when it is too small
+float2* extra_field(const rte_ctx* c, int i) {
+    const size_t f = field_bytes(c);
+    if (!c->extra || (size_t)(i + 1) * f > c->extra_bytes) return nullptr;
+    return (float2*)(c->extra + (size_t)i * f);
+}
+
 // SSP-RK3 (Shu-Osher form, not the paper's integrator):
 //   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2)
 int one_step_ssprk3(rte_ctx* c) {
-    const size_t field = align_up((size_t)c->G * c->Cp * sizeof(float), 256);
-    if (!c->extra) {
-        if (cudaMalloc((void**)&c->extra, field) != cudaSuccess) {
-            cudaGetLastError();
-            return fail(c, RTE_ENOMEM, "rte_step_ssprk3 needs a third state buffer and the device is out of memory");
-        }
-    }
-    float2 *X = c->psi, *Y = c->part, *Z = c->extra;
+    float2* Z = extra_field(c, 0);
+    if (!Z) return fail(c, RTE_EINVAL, "rte_step_ssprk3 needs one state-sized field of extra workspace (rte_set_extra_workspace)");
+    float2 *X = c->psi, *Y = c->part;
     const double tn = (double)c->steps * (double)c->dt, dt = (double)c->dt;
     const size_t n4 = (size_t)c->G * c->Cp / 4;            // Cp is even and records are 8-byte pairs: G*Cp*4 B, /16
     const size_t rem = ((size_t)c->G * c->Cp) % 4;
@@ -580,7 +622,9 @@ cudaError_t upload(T** dst, const std::vector<T>& v, cudaStream_t s) {
 
 // Twiddles and wrapped integer wavenumbers of every supported pencil length -> constant memory, once per device.
 cudaError_t upload_constant_tables(int dev) {
+    static std::mutex mu;
     static bool done[64] = {};
+    std::lock_guard<std::mutex> lock(mu);
     if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
     static const int lens[] = {16, 32, 48, 64, 96, 128, 192, 256, 384, 512};
     std::vector<float2> tw(rtepass::kTableLen);
@@ -602,12 +646,18 @@ cudaError_t upload_constant_tables(int dev) {
     return cudaSuccess;
 }
 
+void drop_graph(rte_ctx* c) {
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+}
+
 void free_ctx(rte_ctx* c) {
     if (!c) return;
     for (int a = 0; a < 3; ++a) {
-        cudaFree(c->ax[a].cpl);
+        cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_op); cudaFree(c->ax[a].tw);
     }
-    cudaFree(c->extra);
+    if (c->graph) cudaGraphExecDestroy(c->graph);
+    cudaFree(c->graph_amp);
+    cudaFree(c->sc); cudaFree(c->partial);
     cudaFree(c->deg); cudaFree(c->ext_of_slot); cudaFree(c->srcw); cudaFree(c->srcS); cudaFree(c->phi_prev);
     cudaFree(c->red);
     delete c;
@@ -617,18 +667,25 @@ int set_source_common(rte_ctx* ctx, const float* w_host, const float* S, bool S_
                       const int ext[3], int kind, float t0, float sig) {
     if (!ctx) return RTE_ESTATE;
     if (kind < 0 || kind > 2) return fail(ctx, RTE_EINVAL, "temporal_kind must be 0, 1 or 2");
-    if (kind == 0) { ctx->src_kind = 0; return RTE_OK; }
+    if (kind == 0) { ctx->src_kind = 0; drop_graph(ctx); return RTE_OK; }
     if (!w_host || !S || !org || !ext) return fail(ctx, RTE_EINVAL, "null source argument");
     if (kind == 2 && !(sig > 0)) return fail(ctx, RTE_EINVAL, "sigma_t must be positive");
     const int n[3] = {ctx->grid.nx, ctx->grid.ny, ctx->grid.nz};
     for (int a = 0; a < 3; ++a)
         if (org[a] < 0 || ext[a] < 1 || org[a] + ext[a] > n[a]) return fail(ctx, RTE_EINVAL, "source box outside the grid");
     const size_t cells = (size_t)ext[0] * ext[1] * ext[2];
+    drop_graph(ctx);
     if (cells > ctx->srcS_cap) {
-        cudaFree(ctx->srcS); ctx->srcS = nullptr; ctx->srcS_cap = 0;
-        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->srcS, cells * sizeof(float)));
+        // the new buffer first: a failure leaves the old source (and its buffer) fully intact
+        float* fresh = nullptr;
+        CUDA_TRY(ctx, cudaMalloc((void**)&fresh, cells * sizeof(float)));
+        ctx->src_kind = 0;                      // until the new footprint is in place no step may read the source
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->srcS);
+        ctx->srcS = fresh;
         ctx->srcS_cap = cells;
     }
+    ctx->src_kind = 0;
     // angular weights in slot order
     std::vector<int> eos, deg;
     rtetab::slot_order(ctx->grid.dim, ctx->N, eos, deg);
@@ -663,45 +720,75 @@ int set_source_common(rte_ctx* ctx, const float* w_host, const float* S, bool S_
 // =====================================================================================================================
 extern "C" {
 
-int rte_num_coeffs(int dim, int N) { return rtetab::num_coeffs(dim, N); }
+int rte_num_coeffs(int dim, int N) { return N > kMaxOrder ? -1 : rtetab::num_coeffs(dim, N); }
 
 int rte_coupling_table(int dim, int N, int axis, double* A_out_host) {
-    const int C = rtetab::num_coeffs(dim, N);
-    if (C < 0 || axis < 0 || axis > 2 || !A_out_host) return RTE_EINVAL;
-    std::vector<double> A[3];
-    rtetab::coupling_real(dim, N, A);
-    std::memcpy(A_out_host, A[axis].data(), (size_t)C * C * sizeof(double));
-    return RTE_OK;
+    return guarded([&]() -> int {
+        const int C = rte_num_coeffs(dim, N);
+        if (C < 0 || axis < 0 || axis > 2 || !A_out_host) return RTE_EINVAL;
+        std::vector<double> A[3];
+        rtetab::coupling_real(dim, N, A);
+        std::memcpy(A_out_host, A[axis].data(), (size_t)C * C * sizeof(double));
+        return RTE_OK;
+    });
 }
 
 int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* cost_host) {
-    if (rtetab::num_coeffs(dim, N) < 0) return RTE_EINVAL;
-    std::vector<int> eos, deg;
-    rtetab::slot_order(dim, N, eos, deg);
-    if (Cp_out) *Cp_out = (int)eos.size();
-    if (ext_of_slot_host) std::memcpy(ext_of_slot_host, eos.data(), eos.size() * sizeof(int));
-    if (cost_host) {
-        const rtetab::PairLayout& L = rtetab::pair_layout(dim, N);
-        cost_host[0] = L.cost0; cost_host[1] = L.cost; cost_host[2] = L.ideal;
-    }
-    return RTE_OK;
+    return guarded([&]() -> int {
+        if (rte_num_coeffs(dim, N) < 0) return RTE_EINVAL;
+        std::vector<int> eos, deg;
+        rtetab::slot_order(dim, N, eos, deg);
+        if (Cp_out) *Cp_out = (int)eos.size();
+        if (ext_of_slot_host) std::memcpy(ext_of_slot_host, eos.data(), eos.size() * sizeof(int));
+        if (cost_host) {
+            const rtetab::PairLayout& L = rtetab::pair_layout(dim, N);
+            cost_host[0] = L.cost0; cost_host[1] = L.cost; cost_host[2] = L.ideal;
+        }
+        return RTE_OK;
+    });
 }
 
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out) {
-    if (!bytes_out || check_grid(grid) != RTE_OK || N < 1) return RTE_EINVAL;
-    const size_t G = (size_t)grid->nx * grid->ny * grid->nz;
-    const size_t Cp = (size_t)padded_coeffs(grid->dim, N);
-    const size_t field = align_up(G * Cp * sizeof(float), 256), map = align_up(G * sizeof(float), 256);
-    *bytes_out = 2 * field + 3 * map;
-    return RTE_OK;
+    return guarded([&]() -> int {
+        if (!bytes_out || check_grid(grid) != RTE_OK || N < 1 || N > kMaxOrder) return RTE_EINVAL;
+        const size_t G = (size_t)grid->nx * grid->ny * grid->nz;
+        const size_t Cp = (size_t)padded_coeffs(grid->dim, N);
+        const size_t field = align_up(G * Cp * sizeof(float), 256), map = align_up(G * sizeof(float), 256);
+        *bytes_out = 2 * field + 3 * map;
+        return RTE_OK;
+    });
 }
 
-int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, float c, const rte_media* media,
-               const rte_pml* pml, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+int rte_extra_workspace_bytes(const rte_grid* grid, int N, int n_fields, size_t* bytes_out) {
+    return guarded([&]() -> int {
+        if (!bytes_out || check_grid(grid) != RTE_OK || N < 1 || N > kMaxOrder || n_fields < 0) return RTE_EINVAL;
+        const size_t G = (size_t)grid->nx * grid->ny * grid->nz;
+        const size_t Cp = (size_t)padded_coeffs(grid->dim, N);
+        *bytes_out = (size_t)n_fields * align_up(G * Cp * sizeof(float), 256);
+        return RTE_OK;
+    });
+}
+
+int rte_stable_dt(int dim, int N, int n_min, float dx, float c, float mu_a_min, float mu_s_min, float g_max,
+                  double* bound_ps_out, double* dt_ps_out) {
+    return guarded([&]() -> int {
+        if (rte_num_coeffs(dim, N) < 0 || n_min < 4 || !(dx > 0) || !(c > 0) || !(mu_a_min >= 0) || !(mu_s_min >= 0) ||
+            !(g_max >= 0 && g_max <= 1))
+            return RTE_EINVAL;
+        double bound = 0;
+        if (!rtetab::stable_dt_bound(dim, N, n_min, dx, c, mu_a_min, mu_s_min, g_max, bound)) return RTE_EUNSUPPORTED;
+        if (bound_ps_out) *bound_ps_out = bound;
+        if (dt_ps_out) *dt_ps_out = 0.5 * bound;
+        return RTE_OK;
+    });
+}
+
+static int create_impl(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, float c, const rte_media* media,
+                       const rte_pml* pml, void* workspace_dev, size_t workspace_bytes, void* cuda_stream, rte_ctx** live) {
     if (!out) return fail(nullptr, RTE_EINVAL, "out is null");
     *out = nullptr;
-    if (check_grid(grid) != RTE_OK) return fail(nullptr, RTE_EINVAL, "unsupported grid (dim 2|3; extents in {16,32,48,64,96,128,192,256,384,512}; nz=1 in 2-D)");
-    if (N < 1 || N > 31) return fail(nullptr, RTE_EINVAL, "N must be in 1..31");
+    if (check_grid(grid) != RTE_OK) return fail(nullptr, RTE_EINVAL, "unsupported grid (dim 2|3; every extent an even 2^a 3^b in [16,1024]; nz=1 in 2-D)");
+    if (N < 1 || N > kMaxOrder) return fail(nullptr, RTE_EINVAL, "N must be in 1..31");
     if (!(dx > 0) || !(dt > 0) || !(c > 0)) return fail(nullptr, RTE_EINVAL, "dx, dt, c must be positive");
     if (!media || !media->mu_a || !media->mu_s || !media->g) return fail(nullptr, RTE_EINVAL, "media pointers are null");
     rte_pml pm{0, 0.f, 0.f};
@@ -724,6 +811,7 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
 
     rte_ctx* ctx = new (std::nothrow) rte_ctx();
     if (!ctx) return fail(nullptr, RTE_ENOMEM, "out of host memory");
+    *live = ctx;
     ctx->grid = *grid; ctx->pml = pm; ctx->N = N;
     ctx->C = rtetab::num_coeffs(grid->dim, N);
     ctx->Cp = padded_coeffs(grid->dim, N);
@@ -749,7 +837,8 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
             int n1 = 0, n2 = 0;
             rtetab::split_of(ext[a], n1, n2);
             if (pass_smem(ext[a], ctx->P, 1, N + 1, a == 0) > kMaxSmem ||
-                (unsigned long long)32 * (unsigned long long)str[a] * (unsigned long long)ctx->P * 8ull >= (1ull << 32)) {
+                (unsigned long long)36 * (unsigned long long)str[a] * (unsigned long long)ctx->P * 8ull >= (1ull << 32)) {
+                *live = nullptr;
                 delete ctx;
                 return fail(nullptr, RTE_EUNSUPPORTED, "grid extent x number of coefficients exceeds one shared-memory pencil tile");
             }
@@ -761,6 +850,7 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
         cudaError_t e__ = (expr);                                                                \
         if (e__ != cudaSuccess) {                                                                \
             fail(nullptr, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e__));                       \
+            *live = nullptr;                                                                     \
             free_ctx(ctx);                                                                       \
             return RTE_ECUDA;                                                                    \
         }                                                                                        \
@@ -775,24 +865,37 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
         rtetab::split_of(T.n, T.N1, T.N2);
         std::vector<std::vector<rtetab::PairEntry>> pe;
         rtetab::pair_coupling(grid->dim, N, a, pe);
-        // weights pre-multiplied by -c dt (eq.(11)); unused entries point at the pair itself with zero weights
-        // -c dt (eq.(11)) times the axis' wavenumber unit and 1/n (the kernel multiplies by the integer wavenumber only)
-        const double mcdt = -(double)c * (double)dt * 6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n;
-        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE);
+        // weights pre-multiplied by the axis' wavenumber unit and 1/n (the kernel multiplies by the integer wavenumber only)
+        // and by -c dt for the time step (eq.(11)) / +1 for the operator L; unused entries: own pair, zero weights
+        const double unit = 6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n;
+        const double scales[2] = {-(double)c * (double)dt * unit, unit};
+        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE), flat_op(flat.size());
         T.maxcnt = 0;
         T.npure = rtetab::pair_layout(grid->dim, N).npure[a];
         for (int p = 0; p < ctx->P; ++p) {
             const int cnt = (int)pe[p].size();
             if (cnt > rtepass::kMaxE) {
+                *live = nullptr;
                 free_ctx(ctx);
                 return fail(nullptr, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
             }
             if (cnt > T.maxcnt) T.maxcnt = cnt;
             for (int e = 0; e < rtepass::kMaxE; ++e)
-                flat[(size_t)p * rtepass::kMaxE + e] =
-                    (e < cnt && pe[p][e].src >= 0) ? CplEntry{(float)(mcdt * pe[p][e].w00), (float)(mcdt * pe[p][e].w11),
-                                       (float)(mcdt * pe[p][e].w01), (float)(mcdt * pe[p][e].w10), pe[p][e].src, 0}
-                            : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
+                for (int v = 0; v < 2; ++v) {
+                    const double m = scales[v];
+                    (v == 0 ? flat : flat_op)[(size_t)p * rtepass::kMaxE + e] =
+                        (e < cnt && pe[p][e].src >= 0) ? CplEntry{(float)(m * pe[p][e].w00), (float)(m * pe[p][e].w11),
+                                           (float)(m * pe[p][e].w01), (float)(m * pe[p][e].w10), pe[p][e].src, 0}
+                                : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
+                }
+        }
+        CREATE_TRY(upload(&T.cpl_op, flat_op, ctx->stream));
+        {
+            std::vector<float> t;
+            rtetab::twiddles(T.n, t);
+            std::vector<float2> tw((size_t)T.n);
+            for (int j = 0; j < T.n; ++j) tw[j] = make_float2(t[2 * j], t[2 * j + 1]);
+            CREATE_TRY(upload(&T.tw, tw, ctx->stream));
         }
         CREATE_TRY(upload(&T.cpl, flat, ctx->stream));
     }
@@ -822,8 +925,27 @@ int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, f
     CREATE_TRY(cudaMemsetAsync(ctx->psi, 0, field, ctx->stream));
     CREATE_TRY(cudaMemsetAsync(ctx->part, 0, field, ctx->stream));
 #undef CREATE_TRY
+    *live = nullptr;
     *out = ctx;
     return RTE_OK;
+}
+
+int rte_create(rte_ctx** out, const rte_grid* grid, int N, float dx, float dt, float c, const rte_media* media,
+               const rte_pml* pml, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+    rte_ctx* live = nullptr;          // the half-built context, so that an exception cannot leak it
+    int rc;
+    try {
+        rc = create_impl(out, grid, N, dx, dt, c, media, pml, workspace_dev, workspace_bytes, cuda_stream, &live);
+    } catch (const std::bad_alloc&) {
+        rc = fail(nullptr, RTE_ENOMEM, "out of host memory");
+        if (live) free_ctx(live);
+        if (out) *out = nullptr;
+    } catch (...) {
+        rc = fail(nullptr, RTE_EINVAL, "unexpected exception in rte_create");
+        if (live) free_ctx(live);
+        if (out) *out = nullptr;
+    }
+    return rc;
 }
 
 void rte_destroy(rte_ctx* ctx) {
@@ -881,21 +1003,87 @@ int rte_reset_time(rte_ctx* ctx) {
 
 int rte_set_source(rte_ctx* ctx, const float* w_host, const float* S_dev, const int box_origin[3],
                    const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps) {
-    return set_source_common(ctx, w_host, S_dev, false, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+    return guarded([&]() -> int {
+        return set_source_common(ctx, w_host, S_dev, false, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+    });
 }
 int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, const int box_origin[3],
                         const int box_extent[3], int temporal_kind, float t0_ps, float sigma_t_ps) {
-    return set_source_common(ctx, w_host, S_host, true, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+    return guarded([&]() -> int {
+        return set_source_common(ctx, w_host, S_host, true, box_origin, box_extent, temporal_kind, t0_ps, sigma_t_ps);
+    });
+}
+
+// ---- CUDA-graph replay for launch-bound (L2-resident) grids -----------------------------------------------------------------
+// A step is 2-3 launches; on a grid whose state lives in L2 the launches, not the kernels, bound the step (cfg0:
+// 11 us/step eager).  kGraphSteps steps (even: the state buffers are back in place) are captured once per context from the
+// SAME launch code and replayed; the time-dependent source amplitude c dt f(t_n) of every captured step is read by
+// the x kernel from a small device table that the host refreshes, stream-ordered, before each replay.
+constexpr int kGraphSteps = 32;
+constexpr size_t kGraphMaxStateBytes = (size_t)24 << 20;   // states up to 24 MB (cfg1: 16.8 MB) are L2-resident
+
+int build_graph(rte_ctx* c) {
+    if (!c->graph_amp) CUDA_TRY(c, cudaMalloc((void**)&c->graph_amp, kGraphSteps * sizeof(float)));
+    const long long steps0 = c->steps, launches0 = c->launches;
+    cudaGraph_t g = nullptr;
+    // captured on a private stream (the caller's may be the legacy default stream, which cannot capture); the
+    // instantiated graph is launched on the caller's stream
+    cudaStream_t cap = nullptr, user = c->stream;
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail(c, RTE_ECUDA, "graph capture: %s", cudaGetErrorString(e)); }
+    c->stream = cap;
+    int rc = RTE_OK;
+    for (int k = 0; k < kGraphSteps && rc == RTE_OK; ++k) rc = one_step(c, nullptr, KIND_STEP, c->graph_amp + k);
+    c->stream = user;
+    e = cudaStreamEndCapture(cap, &g);
+    cudaStreamDestroy(cap);
+    c->steps = steps0; c->launches = launches0;             // nothing ran: capture only recorded the launches
+    if (rc != RTE_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return fail(c, RTE_ECUDA, "graph capture: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&c->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { c->graph = nullptr; return fail(c, RTE_ECUDA, "graph instantiate: %s", cudaGetErrorString(e)); }
+    return RTE_OK;
 }
 
 int rte_step(rte_ctx* ctx, int nsteps) {
     if (!ctx) return RTE_ESTATE;
     if (nsteps < 0) return fail(ctx, RTE_EINVAL, "negative step count");
-    for (int s = 0; s < nsteps; ++s) {
-        const int rc = one_step(ctx);
-        if (rc != RTE_OK) return rc;
-    }
-    return RTE_OK;
+    return guarded([&]() -> int {
+        int left = nsteps;
+        const bool small = (size_t)ctx->G * ctx->Cp * sizeof(float) <= kGraphMaxStateBytes;
+        if (small && left >= kGraphSteps + 1) {
+            if (ctx->launches_warm == 0) {                  // one eager step first: per-device kernel attributes get set
+                const int rc = one_step(ctx);
+                if (rc != RTE_OK) return rc;
+                ctx->launches_warm = 1;
+                --left;
+            }
+            if (!ctx->graph) { const int rc = build_graph(ctx); if (rc != RTE_OK) return rc; }
+            const int per_step = ctx->grid.dim;
+            while (left >= kGraphSteps) {
+                if (ctx->src_kind != 0) {
+                    float amp[kGraphSteps];
+                    for (int k = 0; k < kGraphSteps; ++k)
+                        amp[k] = (float)((double)ctx->c * (double)ctx->dt *
+                                         source_time_factor(ctx, (double)(ctx->steps + k) * (double)ctx->dt));
+                    // pageable source: staged before the call returns, so the stack buffer may go away
+                    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->graph_amp, amp, sizeof(amp), cudaMemcpyHostToDevice, ctx->stream));
+                }
+                CUDA_TRY(ctx, cudaGraphLaunch(ctx->graph, ctx->stream));
+                ctx->steps += kGraphSteps;                  // even count: psi / part are where they were
+                ctx->launches += (long long)kGraphSteps * per_step;
+                left -= kGraphSteps;
+            }
+        }
+        for (int s = 0; s < left; ++s) {
+            const int rc = one_step(ctx);
+            if (rc != RTE_OK) return rc;
+        }
+        ctx->launches_warm = 1;
+        return RTE_OK;
+    });
 }
 
 int rte_step_ssprk3(rte_ctx* ctx, int nsteps) {
@@ -908,12 +1096,150 @@ int rte_step_ssprk3(rte_ctx* ctx, int nsteps) {
     return RTE_OK;
 }
 
+int rte_step_exp(rte_ctx* ctx, int nsteps) {
+    if (!ctx) return RTE_ESTATE;
+    if (nsteps < 0) return fail(ctx, RTE_EINVAL, "negative step count");
+    for (int s = 0; s < nsteps; ++s) {
+        const int rc = one_step(ctx, nullptr, KIND_EXP);
+        if (rc != RTE_OK) return rc;
+    }
+    return RTE_OK;
+}
+
+int rte_set_extra_workspace(rte_ctx* ctx, void* extra_dev, size_t bytes) {
+    if (!ctx) return RTE_ESTATE;
+    if (extra_dev && ((uintptr_t)extra_dev & 255u) != 0) return fail(ctx, RTE_EINVAL, "extra workspace must be 256-byte aligned");
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));       // nothing in flight may still use the old buffers
+    ctx->extra = (char*)extra_dev;
+    ctx->extra_bytes = extra_dev ? bytes : 0;
+    return RTE_OK;
+}
+
+int rte_apply_operator(rte_ctx* ctx, const float* x_dev, float* y_dev) {
+    if (!ctx) return RTE_ESTATE;
+    if (!x_dev || !y_dev) return fail(ctx, RTE_EINVAL, "null field pointer");
+    float2 *X = extra_field(ctx, 0), *Y = extra_field(ctx, 1);
+    if (!Y) return fail(ctx, RTE_EINVAL, "rte_apply_operator needs two state-sized fields of extra workspace (rte_set_extra_workspace)");
+    dim3 grid((unsigned)((ctx->G + 31) / 32), (unsigned)((ctx->Cp + 31) / 32)), block(32, 8);
+    k_import<<<grid, block, 0, ctx->stream>>>((float*)X, x_dev, ctx->ext_of_slot, ctx->G, ctx->Cp);
+    const int rc = euler_update(ctx, X, Y, 0.0, KIND_OPER);
+    if (rc != RTE_OK) return rc;
+    k_export<<<grid, block, 0, ctx->stream>>>(y_dev, (const float*)Y, ctx->ext_of_slot, ctx->G, ctx->Cp);
+    ctx->launches += 2;
+    CUDA_TRY(ctx, cudaGetLastError());
+    return RTE_OK;
+}
+
+// b[cell][slot] = w[slot] S(cell) inside the source box (S is already zero outside Omega), 0 elsewhere
+__global__ void k_source_field(float* __restrict__ b, const float* __restrict__ S, const float* __restrict__ w, int ox, int oy,
+                               int oz, int ex, int ey, int ez, int nx, int ny, long long G, int Cp) {
+    const long long total = G * Cp;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long cell = i / Cp;
+        const int slot = (int)(i - cell * Cp);
+        const int x = (int)(cell % nx);
+        const long long r = cell / nx;
+        const int bx = x - ox, by = (int)(r % ny) - oy, bz = (int)(r / ny) - oz;
+        float v = 0.f;
+        if (bx >= 0 && bx < ex && by >= 0 && by < ey && bz >= 0 && bz < ez)
+            v = w[slot] * S[((size_t)bz * ey + by) * ex + bx];
+        b[i] = v;
+    }
+}
+
+int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int* applications_out, double* relres_out) {
+    using namespace rtesolve;
+    if (!ctx) return RTE_ESTATE;
+    if (restart < 1 || restart > kMaxRestart || !(tol > 0) || max_restarts < 0)
+        return fail(ctx, RTE_EINVAL, "rte_solve_steady: restart in 1..64, tol > 0, max_restarts >= 0");
+    if (ctx->src_kind == 0) return fail(ctx, RTE_EINVAL, "rte_solve_steady needs a source (rte_set_source)");
+    const int m = restart;
+    float2* W = extra_field(ctx, 0);
+    float2* B = extra_field(ctx, 1);
+    float2* V = extra_field(ctx, 2);
+    if (!extra_field(ctx, m + 2))
+        return fail(ctx, RTE_EINVAL, "rte_solve_steady needs restart + 3 state-sized fields of extra workspace (rte_set_extra_workspace)");
+    if (((size_t)ctx->G * ctx->Cp) % 4 != 0) return fail(ctx, RTE_EUNSUPPORTED, "state size not a multiple of 16 bytes");
+    if (!ctx->sc) {
+        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->sc, sizeof(Scalars)));
+        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->partial, (size_t)kRedBlocks * (kMaxRestart + 2) * sizeof(double)));
+    }
+    cudaStream_t st = ctx->stream;
+    Scalars* sc = ctx->sc;
+    double* partial = ctx->partial;
+    const size_t n4 = (size_t)ctx->G * ctx->Cp / 4, stride4 = field_bytes(ctx) / 16;
+    const int NS = kMaxRestart + 1;                            // slot of the norms in a partial-sum row
+    double* hfold = (double*)((char*)sc + offsetof(Scalars, h));
+    const int* halt = (const int*)((char*)sc + offsetof(Scalars, halt));
+    const double* inv = (const double*)((char*)sc + offsetof(Scalars, inv));
+    CUDA_TRY(ctx, cudaMemsetAsync(sc, 0, sizeof(Scalars), st));
+    CUDA_TRY(ctx, cudaMemcpyAsync((char*)sc + offsetof(Scalars, tol), &tol, sizeof(double), cudaMemcpyHostToDevice, st));
+    // b = q (temporal factor 1), ||b||
+    k_source_field<<<grid_for(ctx->G * ctx->Cp, 256), 256, 0, st>>>((float*)B, ctx->srcS, ctx->srcw, ctx->src_org[0], ctx->src_org[1],
+                                                                    ctx->src_org[2], ctx->src_ext[0], ctx->src_ext[1], ctx->src_ext[2],
+                                                                    ctx->grid.nx, ctx->grid.ny, ctx->G, ctx->Cp);
+    k_sub_norm<<<kRedBlocks, kRedThreads, 0, st>>>(nullptr, (const float4*)B, nullptr, n4, partial, NS);
+    k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
+    k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 1);
+    ctx->launches += 4;
+    long long applications = 0;
+    double relres = 0.0;
+    for (int cycle = 0;; ++cycle) {
+        // r_0 = b - L x (true residual), v_0 = r_0 / ||r_0||
+        int rc = euler_update(ctx, ctx->psi, W, 0.0, KIND_OPER);
+        if (rc != RTE_OK) return rc;
+        k_sub_norm<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)V, (const float4*)B, (const float4*)W, n4, partial, NS);
+        k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
+        k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 0);
+        ctx->launches += 3;
+        // the one host read of the cycle: a few scalars (true relative residual, Arnoldi steps done so far)
+        HostView hv{};
+        CUDA_TRY(ctx, cudaMemcpyAsync(&hv, (char*)sc + offsetof(Scalars, bnorm), sizeof(HostView), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        relres = hv.relres;
+        applications = (long long)hv.ktotal + cycle + 1;      // Arnoldi steps + one residual evaluation per cycle
+        if (hv.bnorm == 0.0) {                                 // q = 0: the steady state is psi = 0
+            CUDA_TRY(ctx, cudaMemsetAsync(ctx->psi, 0, field_bytes(ctx), st));
+            relres = 0.0;
+            break;
+        }
+        if (!(relres > tol) || cycle == max_restarts) break;
+        k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)V, (const float4*)V, inv, n4, sc);
+        ctx->launches += 1;
+        for (int k = 0; k < m; ++k) {
+            const float2* vk = (const float2*)((const char*)V + (size_t)k * field_bytes(ctx));
+            float2* vn = (float2*)((char*)V + (size_t)(k + 1) * field_bytes(ctx));
+            rc = euler_update(ctx, vk, W, 0.0, KIND_OPER, nullptr, halt);
+            if (rc != RTE_OK) return rc;
+            k_dots<<<kRedBlocks, kRedThreads, 0, st>>>((const float4*)W, (const float4*)V, stride4, k + 1, n4, partial, sc);
+            k_fold<<<1, 128, 0, st>>>(partial, kRedBlocks, k + 1, hfold, sc);
+            k_update<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)W, (const float4*)V, stride4, k + 1, n4, hfold, partial, NS, sc);
+            k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
+            k_givens<<<1, 1, 0, st>>>(sc, k, NS);
+            k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)vn, (const float4*)W, inv, n4, sc);
+            ctx->launches += 6;
+        }
+        k_solve_y<<<1, 1, 0, st>>>(sc);
+        k_correct<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)ctx->psi, (const float4*)V, stride4, n4, sc);
+        ctx->launches += 2;
+        CUDA_TRY(ctx, cudaGetLastError());
+    }
+    if (applications_out) *applications_out = (int)applications;
+    if (relres_out) *relres_out = relres;
+    ctx->have_prev = false;
+    return RTE_OK;
+}
+
 int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host) {
     if (!ctx) return RTE_ESTATE;
     if (nsteps < 0 || !ms_axis_host) return fail(ctx, RTE_EINVAL, "bad rte_step_profile argument");
     const int naxes = ctx->grid.dim;
-    std::vector<cudaEvent_t> ev((size_t)nsteps * naxes + 1);
-    for (auto& e : ev) CUDA_TRY(ctx, cudaEventCreate(&e));
+    std::vector<cudaEvent_t> ev((size_t)nsteps * naxes + 1, nullptr);
+    for (size_t i = 0; i < ev.size(); ++i)
+        if (cudaEventCreate(&ev[i]) != cudaSuccess) {
+            for (size_t j = 0; j < i; ++j) cudaEventDestroy(ev[j]);
+            return fail(ctx, RTE_ECUDA, "CUDA: %s", "cudaEventCreate failed");
+        }
     int rc = RTE_OK;
     cudaEventRecord(ev[0], ctx->stream);
     for (int s = 0; s < nsteps && rc == RTE_OK; ++s) rc = one_step(ctx, &ev[(size_t)s * naxes + 1]);
@@ -960,7 +1286,7 @@ int rte_fluence_change(rte_ctx* ctx, double* rel_change_out) {
     }
     CUDA_TRY(ctx, cudaMemsetAsync(ctx->red, 0, 2 * sizeof(double), ctx->stream));
     k_fluence_change<<<grid_for(ctx->G, 256), 256, 0, ctx->stream>>>((const float*)ctx->psi, ctx->phi_prev, ctx->red,
-                                                                    nullptr, ctx->grid.dim, ctx->grid.nx, ctx->grid.ny,
+                                                                    ctx->grid.dim, ctx->grid.nx, ctx->grid.ny,
                                                                     ctx->grid.nz, ctx->pml.width, ctx->Cp);
     ctx->launches += 1;
     CUDA_TRY(ctx, cudaGetLastError());

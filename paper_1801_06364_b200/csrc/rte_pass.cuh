@@ -42,7 +42,8 @@ constexpr int kMaxE = 4;   // max source pairs per output pair and axis (checked
 // multiplied by -c dt * 2 pi / (n_a dx) / n_a (Euler step, wavenumber unit and inverse-DFT normalisation of the axis).
 struct alignas(8) CplEntry { float wd0, wd1, ws0, ws1; int src; int pad_; };
 
-enum { MODE_ACC = 0, MODE_FIRST = 1 };
+// MODE_RT (generic kernels): FIRST or ACC decided at run time by PassArgs::first, one instance per pencil length
+enum { MODE_ACC = 0, MODE_FIRST = 1, MODE_RT = 2 };
 
 struct PassArgs {
     // fields
@@ -55,7 +56,13 @@ struct PassArgs {
     const float* ss;        // [G] mu_s in Omega, 0 in the PML
     const float* gm;        // [G] g
     const int* deg;         // [2P] degree l of every slot
-    float cdt;              // c * dt
+    float cdt;              // c * dt  (-1 when the kernels apply the steady-state operator L = T + sigma_l, rte_apply_operator)
+    float ident;            // the Euler diagonal is  s_l = ident - cdt sigma_l : 1 for a time step, 0 for the operator
+    int expo;               // generic kernels only: exponential (integrating-factor) Euler step, s_l = exp(-cdt sigma_l)
+                            // multiplies psi AND the streaming term, the source carries phi_1 (rte_step_exp)
+    int first;              // MODE_RT kernels: 1 = FIRST, 0 = ACC
+    const int* halt;        // optional device flag: non-zero => the launch does nothing (Krylov solver, converged early)
+    const float2* tw;       // generic kernels: forward twiddles exp(-2 pi i j / n) of this axis, n entries (global)
     int nsig;               // N + 1 degrees
     float g_uniform;        // > 0: g is this number in every cell AND the kernel instance is a uniform-g one (UG): the
                             // diagonal table then holds 2 numbers per cell (build_sig); 0: N+1 numbers per cell
@@ -63,6 +70,7 @@ struct PassArgs {
     const float* srcw;      // [2P] angular weight per slot
     int src_org[3], src_ext[3];
     float src_amp;          // c dt f(t_n); 0 => no source this step
+    const float* src_amp_dev;   // optional: device location of c dt f(t_n) (CUDA-graph replay), read when src_amp != 0
     // geometry of this pass (cells)
     int stride_i;           // cell stride along the pencil
     int stride_t;           // cell stride between neighbouring pencils of a tile
@@ -72,7 +80,8 @@ struct PassArgs {
     int nx, ny;
 };
 
-// Supported pencil lengths and where their tables start in the constant arrays.
+// Pencil lengths of the SPECIALISED kernels and where their tables start in the constant arrays (the generic kernels
+// take any even n = 2^a 3^b: twiddles from PassArgs::tw, wavenumbers by integer arithmetic).
 constexpr int kTableLen = 1728;   // 16+32+48+64+96+128+192+256+384+512
 #ifdef __CUDACC__
 __host__ __device__
@@ -192,7 +201,8 @@ struct SourceRow {
         const int by = (int)(pencil % A.ny) - A.src_org[1], bz = (int)(pencil / A.ny) - A.src_org[2];
         if (by < 0 || by >= A.src_ext[1] || bz < 0 || bz >= A.src_ext[2]) return;
         on = true;
-        sw0 = __ldg(A.srcw + 2 * p) * A.src_amp; sw1 = __ldg(A.srcw + 2 * p + 1) * A.src_amp;
+        const float amp = A.src_amp_dev ? __ldg(A.src_amp_dev) : A.src_amp;
+        sw0 = __ldg(A.srcw + 2 * p) * amp; sw1 = __ldg(A.srcw + 2 * p + 1) * amp;
         S = A.srcS + ((size_t)bz * A.src_ext[1] + by) * A.src_ext[0];
         x0 = A.src_org[0]; ext = A.src_ext[0];
     }
@@ -278,7 +288,9 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
 template <int N1, int N2, int QC, int PC, bool STACKED>
 __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int tid, int nt) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
-    constexpr int off = table_offset(N1 * N2);
+    constexpr int n = N1 * N2;
+    constexpr bool CT = QC != 0;                      // specialised kernels: constant-memory tables
+    constexpr int off = CT ? table_offset(n) : 0;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     const int SI = G::SI ? G::SI : Q;
@@ -290,11 +302,19 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
 #pragma unroll
         for (int b = 0; b < N2; ++b) v[b] = row[b * SI];
 #pragma unroll
-        for (int b = 1; b < N2; ++b) { w[b] = c_tw[off + k1 * b]; v[b] = rtefft::cmul(v[b], w[b]); }
+        for (int b = 1; b < N2; ++b) {
+            w[b] = CT ? c_tw[off + k1 * b] : __ldg(A.tw + k1 * b);
+            v[b] = rtefft::cmul(v[b], w[b]);
+        }
         rtefft::dft_fwd<N2>(v);
 #pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2)
-            v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), c_kw[off + k1 + N1 * k2]);   // * i * wrapped(k); 2 pi/(n dx)/n is in the weights
+        for (int k2 = 0; k2 < N2; ++k2) {
+            // * i * wrapped(k), k = k1 + N1 k2: k below n/2, 0 at the Nyquist bin (R5), k - n above; 2 pi/(n dx)/n is in
+            // the weights
+            const int k = k1 + N1 * k2;
+            const float kw = CT ? c_kw[off + k] : (float)(2 * k < n ? k : (2 * k == n ? 0 : k - n));
+            v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kw);
+        }
         rtefft::dft_inv<N2>(v);
 #pragma unroll
         for (int b = 1; b < N2; ++b) v[b] = rtefft::cmulc(v[b], w[b]);
@@ -327,6 +347,8 @@ __device__ __forceinline__ void phase_inv1(const PassArgs& A, float2* tile, int 
 // sigma_l = mu_a + mu_s (1 - g^l) in Omega (eq.(9); g^l by repeated multiplication, R16),
 //         = mu_b for every l in the PML, where the maps hold (mu_b, 0, g) (eq.(12)).
 // Layout sig[l*(ncell+1) + j], j = t*n + i: conflict-free to build (lanes = cells) and to read (lanes = degrees).
+// (General form s_l = ident - c dt sigma_l: ident = 1 for a time step; ident = 0, c dt = -1 gives s_l = sigma_l, the
+// diagonal of the steady-state operator L = T + sigma_l; expo: s_l = exp(-c dt sigma_l), generic kernels only.)
 // Uniform g (A.g_uniform > 0): s_l = 1 - c dt (sa + ss (1 - g^l)) = A + B g^l with A = 1 - c dt (sa + ss), B = c dt ss,
 // so the table holds the float2 (A, B) per cell and every thread keeps g^l of its two slots in registers: one
 // broadcast 8-byte read per element instead of two 4-byte reads, and a quarter of the table-building work.
@@ -343,7 +365,7 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
                 const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
                 sa = __ldg(A.sa + cell); ss = __ldg(A.ss + cell);
             }
-            ab[j] = make_float2(1.f - A.cdt * (sa + ss), A.cdt * ss);
+            ab[j] = make_float2(A.ident - A.cdt * (sa + ss), A.cdt * ss);
         }
         return;
     }
@@ -357,7 +379,8 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
         float pw = 1.f;
         float* dst = sig + j;
         for (int l = 0; l < A.nsig; ++l) {
-            *dst = 1.f - A.cdt * fmaf(ss, 1.f - pw, sa);
+            const float a = A.cdt * fmaf(ss, 1.f - pw, sa);          // c dt sigma_l
+            *dst = A.expo ? expf(-a) : A.ident - a;                  // exponential step: exact decay over the step
             pw *= g;
             dst += ncell + 1;
         }
@@ -426,9 +449,11 @@ __device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int
 }
 
 // ---- tail, generic kernels: coupling from the differentiated pencil + accumulate / integrate -----------------------------
-template <int N1, int N2, int MODE, int E>
+// Exponential step (A.expo; rte_step_exp):  FIRST  new = s (psi + T_x) + phi_1 c dt q,   ACC  new += s T_a,
+// s = exp(-c dt sigma_l) from the table, phi_1 = (1 - s)/(c dt sigma_l) = (1 - s)/(-ln s)  (1 where s = 1).
+template <int N1, int N2, int E>
 __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* tile, const float* sig, long long base, int valid,
-                                             int task, long long pencil0) {
+                                             int task, long long pencil0, bool first) {
     constexpr int n = N1 * N2;
     const int P = A.P;
     const int Q = A.TP * P;
@@ -447,14 +472,15 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
         ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
     }
     const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
-    const float2* lp = (MODE == MODE_FIRST ? A.psi : A.acc) + gi;
+    const float2* lp = (first ? A.psi : A.acc) + gi;
     float2* sp = A.acc + gi;
     float2 r[N1];
 #pragma unroll
     for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
     const float* s0 = sig;
     const float* s1 = sig;
-    if (MODE == MODE_FIRST) {
+    const bool table = first || A.expo;
+    if (table) {
         const int ncell1 = n * A.TP + 1;
         s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
         s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
@@ -469,7 +495,18 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
             T = rtefft::cfma_diag(wd[e].x, wd[e].y, d, T);
             T = rtefft::cfma_swap(ws[e].x, ws[e].y, d, T);
         }
-        if (MODE == MODE_FIRST) {
+        if (A.expo) {
+            const float e0 = s0[a * N2], e1 = s1[a * N2];
+            if (first) {
+                r[a] = make_float2(e0 * (r[a].x + T.x), e1 * (r[a].y + T.y));
+                float2 qv = make_float2(0.f, 0.f);
+                src.add(a * N2 + b, qv);
+                if (qv.x != 0.f) r[a].x = fmaf(e0 < 1.f ? (1.f - e0) / -logf(e0) : 1.f, qv.x, r[a].x);
+                if (qv.y != 0.f) r[a].y = fmaf(e1 < 1.f ? (1.f - e1) / -logf(e1) : 1.f, qv.y, r[a].y);
+            } else {
+                r[a] = rtefft::cfma_diag(e0, e1, T, r[a]);
+            }
+        } else if (first) {
             r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
             src.add(a * N2 + b, r[a]);
         } else {
@@ -494,6 +531,11 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
     static_assert(!TMA || ((32 % (QC ? QC : 1) == 0 && NTC % 32 == 0) ||
                            (NTC % (QC ? QC : 1) == 0 && (QC * N2) % (NTC ? NTC : 1) == 0)),
                   "specialised geometry must let a warp or a CTA round own whole tile rows");
+    // the first tail task runs unguarded (task = tid < Q*N2) and the __syncwarp branch of phase 1 needs whole warps
+    static_assert(!TMA || (QC * N2 >= NTC && (QC * N2) % 32 == 0), "specialised geometry: Q*N2 >= block size, whole warps");
+    static_assert(MODE != MODE_RT || !TMA, "run-time FIRST/ACC is for the generic kernels");
+    if (A.halt != nullptr && *reinterpret_cast<const volatile int*>(A.halt) != 0) return;   // uniform: whole grid
+    const bool first = MODE == MODE_RT ? A.first != 0 : MODE == MODE_FIRST;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
     float2* tile = smem;
@@ -513,7 +555,7 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         __syncthreads();
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
-    if (MODE == MODE_FIRST) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
+    if (first || (!TMA && A.expo)) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
     phase_fwd1<N1, N2, MODE, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
@@ -535,7 +577,7 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         phase_inv1<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
         __syncthreads();
 #pragma unroll 1
-        for (int task = tid; task < Q * N2; task += nt) tail_generic<N1, N2, MODE, E>(A, tile, sig, base, valid, task, pencil0);
+        for (int task = tid; task < Q * N2; task += nt) tail_generic<N1, N2, E>(A, tile, sig, base, valid, task, pencil0, first);
     }
 }
 #endif

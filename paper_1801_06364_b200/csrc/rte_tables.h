@@ -15,7 +15,9 @@
 // Slot 0 is always coefficient 0 (the fluence).
 #pragma once
 #include <cmath>
+#include <complex>
 #include <cstdint>
+#include <limits>
 #include <map>
 #include <mutex>
 #include <utility>
@@ -368,16 +370,6 @@ inline void pair_coupling(int dim, int N, int axis, std::vector<std::vector<Pair
         }
 }
 
-// wavenumbers with the Nyquist bin zeroed (R5), already divided by n (the inverse DFT normalisation)
-inline void kappa_over_n(int n, double dx, std::vector<float>& k) {
-    k.resize(n);
-    const double two_pi = 6.283185307179586476925286766559;
-    for (int j = 0; j < n; ++j) {
-        int f = (2 * j < n) ? j : ((2 * j == n) ? 0 : j - n);
-        k[j] = (float)(two_pi * (double)f / ((double)n * dx) / (double)n);
-    }
-}
-
 // forward twiddles exp(-2 pi i j / n), j = 0..n-1, rounded once from fp64
 inline void twiddles(int n, std::vector<float>& tw /* 2n: re, im */) {
     tw.resize(2 * (size_t)n);
@@ -388,21 +380,139 @@ inline void twiddles(int n, std::vector<float>& tw /* 2n: re, im */) {
     }
 }
 
-// supported pencil lengths and their N1 x N2 split (N1-point transforms in role I, N2-point in role II)
+// Supported pencil lengths: every EVEN n = 2^a 3^b in [16, 1024] (odd lengths have no Nyquist bin and are not offered:
+// reading R5 is stated for even n), with the N1 x N2 split of the two-factor transform (N1-point transforms in role I,
+// N2-point in role II; both are register DFTs of rte_fft.cuh, radix 2/3/4).  X(N1, N2) for the generic kernels'
+// dispatch (rte_lib.cu): one kernel instance per row.
+#define RTE_SPLITS(X)                                                                                                  \
+    X(4, 4) X(6, 3) X(6, 4) X(4, 8) X(6, 6) X(4, 12) X(9, 6) X(8, 8) X(9, 8) X(8, 12) X(12, 9) X(8, 16) X(12, 12)      \
+    X(18, 9) X(12, 16) X(18, 12) X(16, 16) X(18, 16) X(18, 18) X(24, 16) X(24, 18) X(27, 18) X(32, 16) X(24, 24)       \
+    X(27, 24) X(32, 24) X(32, 27) X(36, 27) X(32, 32)
 inline bool split_of(int n, int& N1, int& N2) {
-    switch (n) {
-        case 16: N1 = 4; N2 = 4; return true;
-        case 32: N1 = 4; N2 = 8; return true;
-        case 48: N1 = 4; N2 = 12; return true;
-        case 64: N1 = 8; N2 = 8; return true;
-        case 96: N1 = 8; N2 = 12; return true;
-        case 128: N1 = 8; N2 = 16; return true;
-        case 192: N1 = 12; N2 = 16; return true;
-        case 256: N1 = 16; N2 = 16; return true;
-        case 384: N1 = 24; N2 = 16; return true;
-        case 512: N1 = 32; N2 = 16; return true;
-        default: return false;
+#define RTE_SPLIT_CASE(A, B) if (n == (A) * (B)) { N1 = (A); N2 = (B); return true; }
+    RTE_SPLITS(RTE_SPLIT_CASE)
+#undef RTE_SPLIT_CASE
+    return false;
+}
+
+// ---- forward-Euler stability bound (R10; "time-steps of the order of 100 fs provide stability") ---
+// Eigenvalues of a small dense complex matrix: elementary reduction to Hessenberg form, then shifted QR with deflation
+// (Wilkinson shift, an exceptional shift every 10 sweeps).  a is n x n row-major and is destroyed.
+inline bool eig_complex(std::vector<std::complex<double>>& a, int n, std::vector<std::complex<double>>& lam) {
+    typedef std::complex<double> cd;
+    auto H = [&](int i, int j) -> cd& { return a[(size_t)i * n + j]; };
+    for (int m = 1; m < n - 1; ++m) {                        // Gaussian similarity transforms with pivoting
+        int piv = m;
+        for (int i = m + 1; i < n; ++i) if (std::abs(H(i, m - 1)) > std::abs(H(piv, m - 1))) piv = i;
+        if (std::abs(H(piv, m - 1)) == 0.0) continue;
+        if (piv != m) {
+            for (int j = 0; j < n; ++j) std::swap(H(piv, j), H(m, j));
+            for (int i = 0; i < n; ++i) std::swap(H(i, piv), H(i, m));
+        }
+        for (int i = m + 1; i < n; ++i) {
+            const cd f = H(i, m - 1) / H(m, m - 1);
+            if (f == cd(0, 0)) continue;
+            for (int j = 0; j < n; ++j) H(i, j) -= f * H(m, j);
+            for (int k = 0; k < n; ++k) H(k, m) += f * H(k, i);
+        }
     }
+    lam.assign(n, cd(0, 0));
+    int hi = n - 1, iter = 0;
+    double scale = 0;
+    for (auto& v : a) scale = std::max(scale, std::abs(v));
+    if (scale == 0.0) return true;
+    while (hi >= 0) {
+        int l = hi;
+        while (l > 0) {
+            const double sd = std::abs(H(l - 1, l - 1)) + std::abs(H(l, l));
+            if (std::abs(H(l, l - 1)) <= 1e-15 * (sd > 0 ? sd : scale)) break;
+            --l;
+        }
+        if (l == hi) { lam[hi] = H(hi, hi); --hi; iter = 0; continue; }
+        if (++iter > 400) return false;
+        cd mu;
+        if (iter % 10 == 0) mu = H(hi, hi) + cd(std::abs(H(hi, hi - 1)), 0.0);
+        else {                                              // eigenvalue of the trailing 2x2 closest to H(hi,hi)
+            const cd p = H(hi - 1, hi - 1), q = H(hi - 1, hi), r = H(hi, hi - 1), t = H(hi, hi);
+            const cd tr = p + t, det = p * t - q * r, disc = std::sqrt(tr * tr * 0.25 - det);
+            const cd e1 = tr * 0.5 + disc, e2 = tr * 0.5 - disc;
+            mu = std::abs(e1 - t) < std::abs(e2 - t) ? e1 : e2;
+        }
+        for (int i = l; i <= hi; ++i) H(i, i) -= mu;
+        std::vector<cd> cs(hi - l), sn(hi - l);
+        for (int k = l; k < hi; ++k) {                      // R = G_{hi-1} ... G_l (H - mu)
+            const cd x = H(k, k), y = H(k + 1, k);
+            const double r = std::sqrt(std::norm(x) + std::norm(y));
+            const cd c = r > 0 ? x / r : cd(1, 0), s2 = r > 0 ? y / r : cd(0, 0);
+            cs[k - l] = c; sn[k - l] = s2;
+            for (int j = k; j < n; ++j) {
+                const cd u = H(k, j), v = H(k + 1, j);
+                H(k, j) = std::conj(c) * u + std::conj(s2) * v;
+                H(k + 1, j) = -s2 * u + c * v;
+            }
+        }
+        for (int k = l; k < hi; ++k) {                      // R G_l^H ... G_{hi-1}^H
+            const cd c = cs[k - l], s2 = sn[k - l];
+            const int top = k + 2 <= hi ? k + 2 : hi;
+            for (int i = 0; i <= top; ++i) {
+                const cd u = H(i, k), v = H(i, k + 1);
+                H(i, k) = u * c + v * s2;
+                H(i, k + 1) = -u * std::conj(s2) + v * std::conj(c);
+            }
+        }
+        for (int i = l; i <= hi; ++i) H(i, i) += mu;
+    }
+    return true;
+}
+
+// dt <= -2 Re(lambda)/|lambda|^2 over the eigenvalues of M(k) = -c (i k A_axis + diag sigma_l), sigma_l = mu_a + mu_s (1 - g^l),
+// k along z (3-D) / x (2-D) — rotational invariance — on 200 magnitudes up to the corner Nyquist sqrt(d) (pi/dx)(1 - 2/n).
+// A_axis only links coefficients of one azimuthal order, so M(k) is handled one connected block at a time.
+inline bool stable_dt_bound(int dim, int N, int n, double dx, double c, double mu_a, double mu_s, double g, double& bound) {
+    typedef std::complex<double> cd;
+    const int C = num_coeffs(dim, N);
+    if (C < 0 || n < 4 || !(dx > 0) || !(c > 0)) return false;
+    std::vector<double> A[3];
+    coupling_real(dim, N, A);
+    const std::vector<double>& Az = A[dim == 3 ? 2 : 0];
+    std::vector<int> ext, deg, degc(C, 0);
+    base_slot_order(dim, N, ext, deg);
+    for (size_t s = 0; s < ext.size(); ++s) if (ext[s] >= 0) degc[ext[s]] = deg[s];
+    std::vector<double> sigma(C);
+    for (int i = 0; i < C; ++i) sigma[i] = mu_a + mu_s * (1.0 - std::pow(g, (double)degc[i]));
+    // connected components of the coupling graph
+    std::vector<int> comp(C, -1);
+    std::vector<std::vector<int>> blocks;
+    for (int s0 = 0; s0 < C; ++s0) {
+        if (comp[s0] >= 0) continue;
+        std::vector<int> blk{s0};
+        comp[s0] = (int)blocks.size();
+        for (size_t h = 0; h < blk.size(); ++h)
+            for (int j = 0; j < C; ++j)
+                if (comp[j] < 0 && (Az[(size_t)blk[h] * C + j] != 0.0 || Az[(size_t)j * C + blk[h]] != 0.0)) {
+                    comp[j] = comp[s0];
+                    blk.push_back(j);
+                }
+        blocks.push_back(blk);
+    }
+    const double kmax = std::sqrt((double)dim) * 3.14159265358979323846 / dx * (1.0 - 2.0 / (double)n);
+    bound = std::numeric_limits<double>::infinity();
+    for (int ik = 1; ik <= 200; ++ik) {
+        const double k = kmax * (double)ik / 200.0;
+        for (const auto& blk : blocks) {
+            const int m = (int)blk.size();
+            std::vector<cd> M((size_t)m * m), lam;
+            for (int i = 0; i < m; ++i)
+                for (int j = 0; j < m; ++j)
+                    M[(size_t)i * m + j] = -c * (cd(0.0, k * Az[(size_t)blk[i] * C + blk[j]]) + (i == j ? cd(sigma[blk[i]], 0.0) : cd(0, 0)));
+            if (!eig_complex(M, m, lam)) return false;
+            for (const cd& l : lam) {
+                const double b2 = -2.0 * l.real() / std::norm(l);
+                if (b2 < bound) bound = b2;
+            }
+        }
+    }
+    return true;
 }
 
 }  // namespace rtetab

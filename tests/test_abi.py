@@ -125,3 +125,79 @@ def test_product_does_not_import_oracle():
     for f in ("rte_lib.cu", "rte_pass.cuh", "rte_fft.cuh", "rte_tables.h"):
         text = open(os.path.join(pkg, "csrc", f)).read()
         assert "#include \"../../oracle" not in text and "rte_oracle" not in text
+
+
+# ---- round 2: stability helper, general extents, extra workspace (host only) ---------------------------------------------
+def numpy_stable_dt_bound(dim, N, n, dx, c, mu_a, mu_s, g):
+    """R10 written with numpy.linalg on the quadrature-built coupling matrix (independent of the library's own
+    eigenvalue routine and tables)."""
+    A = quad_coupling(dim, N)[2 if dim == 3 else 0]
+    L = np.array([int(np.floor(np.sqrt(i))) for i in range(A.shape[0])]) if dim == 3 else \
+        np.array([0] + [m for m in range(1, N + 1) for _ in range(2)])
+    sigma = mu_a + mu_s * (1 - g ** L)
+    kmax = np.sqrt(dim) * np.pi / dx * (1 - 2.0 / n)
+    best = np.inf
+    for k in np.linspace(kmax / 200, kmax, 200):
+        lam = np.linalg.eigvals(-c * (1j * k * A + np.diag(sigma)))
+        best = min(best, np.min(-2 * lam.real / np.abs(lam) ** 2))
+    return best
+
+
+@pytest.mark.parametrize("dim,N,n,dx,med", [(2, 3, 64, 0.1, (0.01, 10.0, 0.9)), (3, 3, 128, 0.8, (0.01, 10.0, 0.9)),
+                                            (3, 5, 256, 0.04, (0.01, 5.0, 0.95)), (3, 7, 384, 0.25, (0.01, 3.0, 0.9)),
+                                            (2, 7, 512, 0.05, (0.005, 5.0, 0.9)), (3, 2, 32, 0.3, (0.2, 1.0, 0.0))])
+def test_stable_dt_matches_numpy_eigenvalues(dim, N, n, dx, med):
+    bound, dt = rte.rte_stable_dt(dim, N, n, dx, 0.3, *med)
+    ref = numpy_stable_dt_bound(dim, N, n, dx, 0.3, *med)
+    assert abs(bound - ref) <= 1e-6 * ref          # media arrive as fp32
+    assert dt == 0.5 * bound
+
+
+def test_stable_dt_reproduces_the_survey_table_and_rejects_bad_input():
+    """SURVEY R10 [verified] bounds: cfg0 4.68 fs, cfg2 268 fs, the paper's exp.1 background 66 fs."""
+    assert abs(rte.rte_stable_dt(2, 3, 64, 0.1, 0.3, 0.01, 10.0, 0.9)[0] - 4.68e-3) < 2e-5
+    assert abs(rte.rte_stable_dt(3, 3, 128, 0.8, 0.3, 0.01, 10.0, 0.9)[0] - 0.268) < 1e-3
+    assert abs(rte.rte_stable_dt(3, 21, 64, 50.0 / 64, 0.3, 0.01, 1.0, 0.9)[0] - 0.066) < 1e-3
+    import rte_workloads as wl
+    for name, weak in [("cfg0", (0.01, 10.0, 0.9)), ("cfg1", (0.005, 5.0, 0.9)), ("cfg2", (0.01, 10.0, 0.9)),
+                       ("cfg3", (0.01, 5.0, 0.95)), ("cfg4", (0.01, 3.0, 0.9))]:
+        cfg = wl.CONFIGS[name]
+        assert cfg.dt <= 0.55 * rte.rte_stable_dt(cfg.dim, cfg.N, cfg.nx, cfg.dx, cfg.c, *weak)[0]
+    for bad in [(4, 3, 64, 0.1, 0.3, 0.01, 10.0, 0.9), (3, 0, 64, 0.1, 0.3, 0.01, 10.0, 0.9), (3, 32, 64, 0.1, 0.3, 0.01, 10.0, 0.9),
+                (3, 3, 64, 0.0, 0.3, 0.01, 10.0, 0.9), (3, 3, 64, 0.1, 0.3, 0.01, 10.0, 1.5), (3, 3, 2, 0.1, 0.3, 0.01, 10.0, 0.9)]:
+        with pytest.raises(rte.RteError):
+            rte.rte_stable_dt(*bad)
+
+
+def test_supported_extents_are_the_even_2a3b_numbers():
+    ok = sorted(n for n in range(16, 1025) if n % 2 == 0 and all(p in (2, 3) for p in _prime_factors(n)))
+    assert len(ok) == 29 and ok[:6] == [16, 18, 24, 32, 36, 48] and ok[-3:] == [864, 972, 1024]
+    for n in range(2, 1100):
+        try:
+            rte.rte_workspace_bytes((2, n, 16, 1), 1)
+            accepted = True
+        except rte.RteError:
+            accepted = False
+        assert accepted == (n in ok), n
+
+
+def _prime_factors(n):
+    out, p = [], 2
+    while n > 1:
+        while n % p == 0:
+            out.append(p)
+            n //= p
+        p += 1
+    return out
+
+
+def test_extra_workspace_bytes_and_order_cap():
+    one = rte.rte_extra_workspace_bytes((3, 32, 32, 32), 3, 1)
+    assert one >= 32 ** 3 * 16 * 4 and one % 256 == 0
+    assert rte.rte_extra_workspace_bytes((3, 32, 32, 32), 3, 33) == 33 * one
+    assert rte.rte_extra_workspace_bytes((3, 32, 32, 32), 3, 0) == 0
+    assert rte.rte_num_coeffs(3, 31) == 1024 and rte.rte_num_coeffs(3, 32) < 0 and rte.rte_num_coeffs(3, 50000) < 0
+    with pytest.raises(rte.RteError):
+        rte.rte_coupling_table(3, 50000, 0)
+    with pytest.raises(rte.RteError):
+        rte.rte_storage_layout(3, 40)

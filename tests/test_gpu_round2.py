@@ -1,0 +1,196 @@
+"""GPU parity for the round-2 rows (SURVEY 8(b) general extents, 8(f1) operator + Krylov steady state, 8(f2) exponential
+step, CUDA-graph stepping): the CUDA path through the C ABI against the fp64 oracle on the same seeded fp32 inputs.
+Same acceptance as test_gpu_parity.py.  Run with -m gpu."""
+import numpy as np
+import pytest
+import torch
+
+import paper_1801_06364_b200 as rte
+import rte_workloads as wl
+from oracle import rte_oracle as orc
+from test_gpu_parity import DEV, assert_parity, dev, field_errors, gpu_create, gpu_state, make_oracle, run_both
+
+pytestmark = pytest.mark.gpu
+
+
+def random_case(dim, nx, ny, nz, N, dx=0.2, dt=0.002, W=3, seed=0):
+    rng = np.random.default_rng(seed + nx * 7 + ny * 3 + nz + N)
+    cfg = wl.Config("rand", dim, nx, ny, nz, N, dx, dt, 0.3, 3, (W, 0.01, 2.0), "random", "box", 0)
+    mu_a = rng.uniform(0.01, 0.5, cfg.shape).astype(np.float32)
+    mu_s = rng.uniform(2.0, 20.0, cfg.shape).astype(np.float32)
+    g = rng.uniform(0.7, 0.95, cfg.shape).astype(np.float32)
+    ext = (5, 4, 3 if dim == 3 else 1)
+    src = dict(w=rng.standard_normal(cfg.C).astype(np.float32), S=rng.standard_normal(ext[::-1]).astype(np.float32),
+               origin=(1, 2, 4 if dim == 3 else 0), extent=ext, kind=1, t0=0.0, sigma_t=1.0)
+    return cfg, mu_a, mu_s, g, src
+
+
+# ---- every pencil length the generic kernels add this round (even 2^a 3^b), on every axis position ------------------------
+NEW_SHAPES_3D = [(18, 24, 36, 3), (36, 18, 24, 2), (24, 36, 18, 1), (54, 16, 72, 3), (72, 54, 16, 2), (16, 72, 54, 3),
+                 (108, 16, 16, 3), (16, 144, 16, 2), (16, 16, 162, 3), (216, 16, 16, 1), (16, 288, 16, 3), (16, 16, 324, 2),
+                 (432, 16, 16, 3), (16, 486, 16, 1), (16, 16, 576, 3), (648, 16, 16, 2), (16, 768, 16, 3), (16, 16, 864, 1),
+                 (972, 16, 16, 3), (16, 1024, 16, 2), (16, 16, 1024, 3)]
+
+
+@pytest.mark.parametrize("nx,ny,nz,N", NEW_SHAPES_3D)
+def test_general_extents_3d(nx, ny, nz, N):
+    cfg, mu_a, mu_s, g, src = random_case(3, nx, ny, nz, N)
+    got, ref, _ = run_both(cfg, mu_a, mu_s, g, wl.random_state(cfg, seed=N), src, cfg.steps)
+    assert_parity(got, ref, f"{nx}x{ny}x{nz} P{N}")
+
+
+@pytest.mark.parametrize("nx,ny,N", [(18, 54, 3), (144, 24, 2), (1024, 16, 3), (36, 972, 1), (768, 108, 4)])
+def test_general_extents_2d(nx, ny, N):
+    cfg, mu_a, mu_s, g, src = random_case(2, nx, ny, 1, N, dx=0.1, dt=0.001, W=4)
+    got, ref, _ = run_both(cfg, mu_a, mu_s, g, wl.random_state(cfg, seed=N), src, 4)
+    assert_parity(got, ref, f"{nx}x{ny} P{N}")
+
+
+def test_unsupported_extents_are_rejected():
+    for n in (20, 27, 81, 100, 2048):
+        with pytest.raises(rte.RteError) as e:
+            rte.rte_create((3, n, 16, 16), 1, 0.1, 0.001, 0.3, 0.01, 10.0, 0.9)
+        assert e.value.code == rte.RTE_EINVAL
+    with pytest.raises(rte.RteError) as e:      # one pencil of all coefficients must fit a shared-memory tile
+        rte.rte_create((3, 1024, 16, 16), 9, 0.1, 0.001, 0.3, 0.01, 10.0, 0.9)
+    assert e.value.code == rte.RTE_EUNSUPPORTED
+
+
+# ---- the steady-state operator and the device-resident GMRES -------------------------------------------------
+@pytest.mark.parametrize("shape,N,maps", [((32, 48, 16), 3, True), ((64, 64, 1), 4, True), ((128, 128, 128), 3, False),
+                                          ((18, 24, 36), 2, True)])
+def test_apply_operator_vs_oracle(shape, N, maps):
+    """y = L x = T[x] + sigma_l x on random x: generic kernels (maps, PML), 2-D, and the specialised cfg2 kernels with
+    scalar media (the uniform-g instance) at 128^3."""
+    nx, ny, nz = shape
+    dim = 3 if nz > 1 else 2
+    cfg, mu_a, mu_s, g, _ = random_case(dim, nx, ny, nz, N, W=4)
+    if not maps:
+        mu_a, mu_s, g = 0.02, 8.0, 0.85
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    x = wl.random_state(cfg, seed=11)
+    xd = dev(x)
+    yd = torch.empty_like(xd)
+    rte.rte_set_state(ctx, dev(wl.random_state(cfg, seed=12)))
+    before = gpu_state(ctx, cfg)
+    rte.rte_apply_operator(ctx, xd, yd)
+    rte.rte_sync(ctx)
+    got = yd.cpu().numpy().astype(np.float64)
+    ref = make_oracle(cfg, mu_a, mu_s, g).apply_operator(x)
+    assert_parity(got, ref, f"operator {shape} P{N}")
+    assert np.array_equal(before, gpu_state(ctx, cfg)) and rte.rte_time_ps(ctx) == 0.0     # state and clock untouched
+
+
+def steady_case(n, N, W, n_incl, dx):
+    cfg = wl.reduced(wl.CONFIGS["cfg3"], n, pml_width=W, dx=dx)
+    cfg = wl.replace(cfg, n_inclusions=n_incl, N=N)
+    return cfg, wl.media_maps(cfg), wl.source_term(cfg)
+
+
+@pytest.mark.parametrize("n,N,W,dx,otol", [(32, 3, 5, 0.16, 1e-10), (48, 5, 6, 0.2, 1e-8)])
+def test_solve_steady_vs_oracle(n, N, W, dx, otol):
+    """Converged steady state of the cfg3 structure (ellipsoid inclusions with varying mu_a, mu_s, g; PML; constant
+    collimated source): device GMRES(30) in fp32 against the oracle's fp64 GMRES solved to 1e-10 (32^3 P_3) / 1e-8
+    (48^3 P_5: the size the plain oracle finishes in minutes)."""
+    cfg, (mu_a, mu_s, g), src = steady_case(n, N, W, 8, dx)
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    rte.rte_set_source(ctx, src["w"], dev(src["S"]), src["origin"], src["extent"], 1)
+    napp, rr = rte.rte_solve_steady(ctx, restart=30, tol=2e-6, max_restarts=60)
+    got = gpu_state(ctx, cfg)
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_source(src["w"], src["S"], src["origin"], src["extent"], 1)
+    onapp, orr = o.solve_steady(restart=30 if n <= 32 else 60, tol=otol, max_restarts=200)
+    ref = o.get_state()
+    assert orr <= otol and rr <= 2e-6, (rr, orr)
+    assert 10 < napp < 4 * onapp
+    assert_parity(got, ref, f"steady {n}^3 P{N} ({napp} applications, oracle {onapp})")
+    # the oracle's own true residual of the GPU field (fp64 operator on the fp32 solution)
+    q = o.source_field()
+    assert np.linalg.norm(o.apply_operator(got) - q) <= 1e-4 * np.linalg.norm(q)
+
+
+def test_solve_steady_uniform_source_breakdown_and_restart_from_solution():
+    """Uniform source, uniform periodic medium: the Krylov space is exhausted after a few steps (happy breakdown) and
+    psi_c = q_c / sigma_l exactly (P7's closed form); solving again from the solution does (almost) no work."""
+    cfg = wl.Config("uni", 3, 16, 16, 16, 2, 0.1, 0.01, 0.3, 1, (0, 0.0, 0.0), "homogeneous", "box", 0)
+    ctx = rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, 0.5, 3.0, 0.5)
+    w = (np.arange(1, cfg.C + 1) * 0.25).astype(np.float32)
+    rte.rte_set_source(ctx, w, dev(np.full(cfg.shape, 2.0, np.float32)), (0, 0, 0), (16, 16, 16), 1)
+    napp, rr = rte.rte_solve_steady(ctx, restart=12, tol=1e-6, max_restarts=5)
+    L = np.array([0, 1, 1, 1, 2, 2, 2, 2, 2])
+    fixed = 2.0 * w / (0.5 + 3.0 * (1 - 0.5 ** L))
+    got = gpu_state(ctx, cfg)
+    assert rr <= 1e-6 and napp <= 12
+    assert np.abs(got - fixed[:, None, None, None]).max() <= 2e-6 * fixed.max()
+    napp2, rr2 = rte.rte_solve_steady(ctx, restart=12, tol=1e-6, max_restarts=5)
+    assert napp2 == 1 and rr2 <= 1e-6
+    with pytest.raises(rte.RteError):
+        rte.rte_solve_steady(ctx, restart=65)
+    rte.rte_set_source(ctx, None, None, None, None, 0)
+    with pytest.raises(rte.RteError):
+        rte.rte_solve_steady(ctx, restart=8)
+
+
+# ---- exponential (integrating-factor) Euler step -------------------------------------------------------------
+@pytest.mark.parametrize("shape,N,dt", [((32, 48, 16), 3, 0.004), ((64, 96, 1), 4, 0.002), ((128, 16, 16), 2, 0.05)])
+def test_exp_step_vs_oracle(shape, N, dt):
+    nx, ny, nz = shape
+    dim = 3 if nz > 1 else 2
+    cfg, mu_a, mu_s, g, src = random_case(dim, nx, ny, nz, N, dt=dt, W=4)
+    if dt >= 0.05:                       # stiff diagonal (c dt sigma up to ~3: eq.(11) would diverge), weak streaming
+        cfg = wl.replace(cfg, dx=2.0)
+    src = dict(src, kind=2, t0=3 * dt, sigma_t=2 * dt)
+    psi0 = wl.random_state(cfg, seed=N)
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    rte.rte_set_state(ctx, dev(psi0))
+    rte.rte_set_source(ctx, src["w"], dev(src["S"]), src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_state(psi0)
+    o.set_source(src["w"], src["S"], src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    rte.rte_step_exp(ctx, 6)
+    o.step_exp(6)
+    assert_parity(gpu_state(ctx, cfg), o.get_state(), f"exp step {shape} P{N}")
+    assert abs(rte.rte_time_ps(ctx) - 6 * dt) < 1e-6
+
+
+def test_exp_step_uniform_decay_exact_on_device():
+    """P16 on the device: a uniform field decays as exp(-c sigma_l t) with no O(dt) error at c dt sigma_l ~ 1."""
+    cfg = wl.Config("uni", 3, 16, 16, 16, 3, 0.1, 0.35, 0.3, 1, (0, 0.0, 0.0), "homogeneous", "none", 0)
+    ctx = rte.rte_create(cfg.grid, cfg.N, cfg.dx, cfg.dt, cfg.c, 0.013, 9.0, 0.87)
+    amp = (1.0 + np.arange(cfg.C)).astype(np.float32)
+    rte.rte_set_state(ctx, dev(np.broadcast_to(amp[:, None, None, None], (cfg.C,) + cfg.shape).copy()))
+    rte.rte_step_exp(ctx, 11)
+    L = np.array([int(np.floor(np.sqrt(c))) for c in range(cfg.C)])
+    ex = amp * np.exp(-0.3 * (0.013 + 9.0 * (1 - 0.87 ** L)) * 11 * 0.35)
+    got = gpu_state(ctx, cfg)
+    assert np.abs(got / ex[:, None, None, None] - 1).max() < 2e-5
+
+
+# ---- CUDA-graph replay on L2-resident grids --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim", [2, 3])
+def test_graph_stepping_is_bit_identical_to_eager(dim):
+    """rte_step(n) with n > 32 on a small grid replays captured launches; the time-dependent source amplitude comes from
+    a device table.  Same bits as n single eager steps, and both match the oracle."""
+    nz = 32 if dim == 3 else 1
+    cfg, mu_a, mu_s, g, src = random_case(dim, 64, 48, nz, 3, dx=0.1, dt=0.001, W=4)
+    src = dict(src, kind=2, t0=0.04, sigma_t=0.02)
+    psi0 = wl.random_state(cfg, seed=5)
+    states = []
+    for mode in ("graph", "eager"):
+        ctx = gpu_create(cfg, mu_a, mu_s, g)
+        rte.rte_set_state(ctx, dev(psi0))
+        rte.rte_set_source(ctx, src["w"], dev(src["S"]), src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+        if mode == "graph":
+            rte.rte_step(ctx, 70)       # 1 eager + 2 x 32 replayed + 5 eager
+            rte.rte_step(ctx, 37)       # 1 x 32 replayed + 5 eager
+        else:
+            for _ in range(107):
+                rte.rte_step(ctx, 1)
+        assert abs(rte.rte_time_ps(ctx) - 107 * cfg.dt) < 1e-6          # dt is an fp32 argument
+        states.append(gpu_state(ctx, cfg))
+    assert np.array_equal(states[0], states[1])
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_state(psi0)
+    o.set_source(src["w"], src["S"], src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    o.step(107)
+    assert_parity(states[0], o.get_state(), "graph stepping")
