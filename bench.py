@@ -53,14 +53,25 @@ def parse_args(argv=None):
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD,
                     choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4", "paper_exp1", "paper_exp2"])
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft_literal"],
+                    help="ours: the product; reference: the fp64 oracle on the host cores; cufft_literal: the paper's own "
+                         "GPU structure (3-D cuFFT per complex field + eq.(10) k-space kernel + pointwise kernel) as a timed "
+                         "reference point on the same box (SURVEY 8(f4), 3-D workloads)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
     ap.add_argument("--no-others", action="store_true", help="skip the short cfg2/cfg3 side measurements")
+    ap.add_argument("--oracle-full-size", action="store_true",
+                    help="time the oracle leg (cpu_baseline / --impl reference) on the FULL workload for 2 steps instead of the "
+                         "bounded sample (cfg2: seconds, cfg3: ~1 min on 16 cores; cfg4 needs > 100 GB of host RAM and "
+                         "minutes per step and is not offered)")
+    ap.add_argument("--krylov-plain", action="store_true",
+                    help="with --steady-state: also run unpreconditioned GMRES(30) on L psi = q (minutes on cfg3)")
     ap.add_argument("--steady-state", action="store_true",
                     help="also run the workload to the steady-state criterion of configs[3] (DESIGN.md R17) with the "
                          "SSP-RK3 integrator at dt = 0.3 dx/c and report steps / seconds (constant-source workloads)")
     a = ap.parse_args(argv)
+    global FULL_SIZE_ORACLE
+    FULL_SIZE_ORACLE = bool(a.oracle_full_size)
     if a.steps is None:
         a.steps = DEFAULT_STEPS[a.workload]
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else max(a.warmup, 0)
@@ -79,12 +90,19 @@ def hbm_peak():
 # ---------------------------------------------------------------------------------------------------------------------
 # algorithmic bytes: S = 4*C*G bytes is one fp32 state
 # ---------------------------------------------------------------------------------------------------------------------
+def first_axis(cfg):
+    """Axis of the FIRST pass (the one that stores the new buffer; the others add to it): x.  (FIRST on z, whose coupling
+    has the smaller fan-in, was measured and rejected: DESIGN.md 6.)"""
+    return 0
+
+
 def algorithmic_bytes(cfg):
-    """Bytes each per-axis kernel must move per launch, and per step.  x pass: read psi and the three per-cell
+    """Bytes each per-axis kernel must move per launch, and per step.  FIRST pass: read psi and the three per-cell
     coefficient maps (12 B/cell), write the new buffer (2 S + 12 G); every other pass: read psi, read + write the new
     buffer (the reductions are read-modify-write in the L2: 3 S).  2-D has no z pass."""
     S = 4 * cfg.C * cfg.G
-    per_axis = [2 * S + 12 * cfg.G, 3 * S, 3 * S] if cfg.dim == 3 else [2 * S + 12 * cfg.G, 3 * S, 0]
+    per_axis = [3 * S, 3 * S, 3 * S if cfg.dim == 3 else 0]
+    per_axis[first_axis(cfg)] = 2 * S + 12 * cfg.G
     return per_axis, sum(per_axis)
 
 
@@ -149,8 +167,13 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------------
 # the oracle legs (the only code in this file that touches oracle/)
 # ---------------------------------------------------------------------------------------------------------------------
+FULL_SIZE_ORACLE = False
+
+
 def oracle_sample_config(wl, cfg):
     n, W, steps = ORACLE_SAMPLE[cfg.name]
+    if FULL_SIZE_ORACLE and cfg.name != "cfg4":
+        return cfg, 2, f"{cfg.name} at FULL size ({cfg.nx}^{cfg.dim}, C={cfg.C}), 2 steps"
     if n >= max(cfg.nx, cfg.ny, cfg.nz):
         return cfg, min(steps, cfg.steps), f"{cfg.name} at full size, {min(steps, cfg.steps)} step(s)"
     small = wl.reduced(cfg, n, pml_width=W)
@@ -314,9 +337,9 @@ def measure_workload(rte, wl, cfg, torch, dev, steps, warmup, dist=None, sampler
 def roofline_of(cfg, res, peak, peak_kind):
     per_axis, per_step = algorithmic_bytes(cfg)
     naxes = cfg.dim
-    names = ["pass_x (first: coupling, DFT-ik-IDFT, sigma_l, PML, source -> stores the new buffer)",
-             "pass_y (coupling, DFT-ik-IDFT -> vector reductions into the new buffer)",
-             "pass_z (coupling, DFT-ik-IDFT -> vector reductions into the new buffer)"]
+    fa = first_axis(cfg)
+    names = [f"pass_{'xyz'[a]} (" + ("first: coupling, DFT-ik-IDFT, sigma_l, PML, source -> stores the new buffer)" if a == fa
+                                     else "coupling, DFT-ik-IDFT -> vector reductions into the new buffer)") for a in range(3)]
     dom = max(range(naxes), key=lambda a: res["ms_axis"][a])
     ach = per_axis[dom] / (res["ms_axis"][dom] * 1e-3) / 1e9
     kernels = []
@@ -354,7 +377,7 @@ def job_value(cfg, steps, world, ms):
     return cfg.C * cfg.G * steps * world / (ms * 1e-3)
 
 
-def steady_state_run(rte, wl, cfg, torch, dev, max_steps=20000, tol=1e-6):
+def steady_state_run(rte, wl, cfg, torch, dev, max_steps=20000, tol=1e-6, plain_krylov=False):
     """configs[3]: "stepped to steady state (until relative change in l=0 fluence < 1e-6 per 100 steps)" (R17).  With the
     paper's forward Euler the stable dt of cfg3 (0.1 fs) makes that 1e5-1e6 steps; the SSP-RK3 step (not the
     paper's integrator) is stable at dt = 0.3 dx/c, hundreds of times larger, and gets there in seconds."""
@@ -377,10 +400,102 @@ def steady_state_run(rte, wl, cfg, torch, dev, max_steps=20000, tol=1e-6):
         if change < tol:
             break
     sec = time.perf_counter() - t0
-    return {"integrator": "ssprk3 (non-paper)", "dt_ps": dt, "euler_dt_ps": cfg.dt, "steps": steps, "seconds": sec,
-            "simulated_ps": steps * dt, "criterion": f"relative L2 change of the fluence over Omega per 100 steps < {tol:g}",
-            "final_change": change, "converged": bool(change < tol),
-            "change_every_1000_steps": [hist[i] for i in range(9, len(hist), 10)][:20]}
+    rk = {"integrator": "ssprk3 (non-paper)", "dt_ps": dt, "euler_dt_ps": cfg.dt, "steps": steps, "seconds": sec,
+          "operator_applications": 3 * steps,
+          "simulated_ps": steps * dt, "criterion": f"relative L2 change of the fluence over Omega per 100 steps < {tol:g}",
+          "final_change": change, "converged": bool(change < tol),
+          "change_every_1000_steps": [hist[i] for i in range(9, len(hist), 10)][:20]}
+    phi_rk = torch.empty(cfg.shape, dtype=torch.float32, device=dev)
+    rte.rte_fluence(ctx, phi_rk)
+    rte.rte_sync(ctx)
+    del ctx
+    torch.cuda.empty_cache()
+    # SURVEY 8(f1) / PAPER.md:109,195: the same steady state by the device-resident Krylov solver, L psi = q
+    out = {"ssprk3": rk}
+    dtp = 0.3 * cfg.dx / cfg.c
+    variants = [("gmres20_rk3x8", dict(restart=20, tol=1e-6, max_restarts=200, precond_steps=8, precond_dt_ps=dtp)),
+                ("gmres20_rk3x16", dict(restart=20, tol=1e-6, max_restarts=200, precond_steps=16, precond_dt_ps=dtp)),
+                ("gmres10_rk3x32", dict(restart=10, tol=1e-6, max_restarts=200, precond_steps=32, precond_dt_ps=dtp))]
+    if plain_krylov:
+        variants.append(("gmres30_plain", dict(restart=30, tol=1e-5, max_restarts=400)))
+    for name, kw in variants:
+        ctx = make_context(rte, wl, cfg, torch, dev)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        napp, rr = rte.rte_solve_steady(ctx, **kw)
+        rte.rte_sync(ctx)
+        ksec = time.perf_counter() - t0
+        phi_k = torch.empty(cfg.shape, dtype=torch.float32, device=dev)
+        rte.rte_fluence(ctx, phi_k)
+        rte.rte_sync(ctx)
+        diff = float((phi_k - phi_rk).norm() / phi_rk.norm())
+        out[name] = {"solver": "rte_solve_steady: device-resident restarted GMRES" +
+                               (" on (I - Phi^s) psi = Phi^s(0; q), Phi = SSP-RK3 step" if kw.get("precond_steps") else " on L psi = q"),
+                     **{k: v for k, v in kw.items()}, "seconds": ksec, "operator_sweeps": napp,
+                     "true_relative_residual": rr, "converged": bool(rr <= kw["tol"]),
+                     "extra_workspace_fields": kw["restart"] + 3 + (3 if kw.get("precond_steps") else 0),
+                     "fluence_rel_l2_difference_from_the_time_stepped_state": diff}
+        del ctx, phi_k
+        torch.cuda.empty_cache()
+    return out
+
+
+def run_cufft_literal(args, wl, cfg):
+    """The paper's structure on this box: a reference point for DESIGN.md 7, not the product."""
+    import torch
+    if cfg.dim != 3:
+        print(json.dumps({"impl": "cufft_literal", "unavailable": "the literal variant is 3-D only"}), flush=True)
+        return 0
+    import paper_1801_06364_b200 as rte
+    from baseline import cufft_literal as cl
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda:0")
+    peak, peak_kind = hbm_peak()
+    mu_a, mu_s, g = device_media(rte, wl, cfg, torch, dev)
+    full = lambda v: v if isinstance(v, torch.Tensor) else torch.full(cfg.shape, float(v), dtype=torch.float32, device=dev)
+    mu_b = torch.empty(cfg.shape, dtype=torch.float32, device=dev)
+    inside = torch.empty(cfg.shape, dtype=torch.uint8, device=dev)
+    rte.rte_pml_profile(cfg.grid, cfg.pml, mu_b, inside)
+    torch.cuda.synchronize()
+    sa = torch.where(inside.bool(), full(mu_a), mu_b)
+    ss = torch.where(inside.bool(), full(mu_s), torch.zeros_like(mu_b))
+    gm = full(g).clone()
+    del mu_b, inside, mu_a, mu_s, g
+    sol = cl.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.N, cfg.dx, cfg.dt, cfg.c, sa, ss, gm)
+    psi = device_initial_state(wl, cfg, torch, dev)
+    pc = cl.real_to_complex(psi)
+    del psi
+    sol.set_state(pc)
+    del pc
+    torch.cuda.empty_cache()
+    sol.step(args.warmup)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    l0 = sol.own_kernel_launches()
+    e0.record()
+    sol.step(args.steps)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    finite = bool(torch.isfinite(torch.view_as_real(sol.get_state()[0])).all().item())
+    S = 4 * cfg.C * cfg.G
+    # its own minimal traffic on the same accounting (S = one REAL fp32 state; its fields are complex, 2 S per sweep):
+    # forward 3-D FFT >= read + write (4 S), k-space kernel read + write (4 S), inverse FFT (4 S), pointwise read psi,
+    # read T, write psi (6 S) = 18 S when every 3-D FFT makes ONE pass over its field (it makes more)
+    line = {"impl": "cufft_literal", "metric": METRIC, "value": cfg.C * cfg.G * args.steps / (ms * 1e-3), "unit": UNIT,
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c64", "data": "synthetic",
+            "config": {"workload": cfg.name, "structure": "PAPER.md:123-131: 3-D C2C cuFFT per complex field, eq.(10) in k-space, "
+                       "inverse cuFFT, pointwise potential + eq.(11); no source term", "complex_fields": cfg.C,
+                       "device_bytes": sol.device_bytes()},
+            "gpu_launches": sol.own_kernel_launches() - l0, "cufft_execs_per_step": 2 * cfg.C, "finite": finite,
+            "traffic_model_bytes_per_step_lower_bound": 18 * S,
+            "effective_gbs_of_the_products_8S_model": (8 * S + 12 * cfg.G) / (ms / args.steps * 1e-3) / 1e9,
+            "hbm_peak_gbs": peak, "peak_kind": peak_kind}
+    print(json.dumps(line), flush=True)
+    return 0
 
 
 def run_ours(args, wl, cfg):
@@ -482,6 +597,20 @@ def run_ours(args, wl, cfg):
         line["ssprk3"] = {"ms_per_step": rk_ms, "steps": k, "algorithmic_bytes_per_step": rk_bytes,
                           "frac_of_hbm_roofline": rk_bytes / (rk_ms * 1e-3) / 1e9 / peak,
                           "note": "non-paper integrator; stable up to dt ~ dx/c, i.e. tens of times the Euler dt"}
+        rte.rte_set_extra_workspace(ctx, 0)
+        torch.cuda.empty_cache()
+        # side measurement: exponential Euler step, generic kernels, diagonal table in every pass
+        rte.rte_step_exp(ctx, 1)
+        torch.cuda.synchronize()
+        e0.record()
+        rte.rte_step_exp(ctx, k)
+        e1.record()
+        torch.cuda.synchronize()
+        ex_ms = e0.elapsed_time(e1) / k
+        ex_bytes = roof["whole_step"]["algorithmic_bytes"] + 2 * 12 * cfg.G * (cfg.dim - 1)
+        line["exp_step"] = {"ms_per_step": ex_ms, "steps": k, "algorithmic_bytes_per_step": ex_bytes,
+                            "frac_of_hbm_roofline": ex_bytes / (ex_ms * 1e-3) / 1e9 / peak,
+                            "note": "rte_step_exp: exact diagonal exp(-c dt sigma_l); runs on the generic kernels"}
 
     if not args.no_others and world == 1 and cfg.name == DEFAULT_WORKLOAD:
         del res, ctx
@@ -508,7 +637,7 @@ def run_ours(args, wl, cfg):
             except NameError:
                 pass
             torch.cuda.empty_cache()
-            line["steady_state"] = steady_state_run(rte, wl, cfg, torch, dev)
+            line["steady_state"] = steady_state_run(rte, wl, cfg, torch, dev, plain_krylov=args.krylov_plain)
 
     if not args.no_cpu_baseline:
         sec, units_small, cores, what = time_oracle(wl, cfg)
@@ -527,6 +656,8 @@ def main(argv=None):
     cfg = wl.CONFIGS[args.workload] if args.workload in wl.CONFIGS else wl.PAPER_EXPERIMENTS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl, cfg)
+    if args.impl == "cufft_literal":
+        return run_cufft_literal(args, wl, cfg)
     return run_ours(args, wl, cfg)
 
 

@@ -94,7 +94,7 @@ int rte_storage_layout(int dim, int N, int* Cp_out, int* ext_of_slot_host, int* 
 int rte_workspace_bytes(const rte_grid* grid, int N, size_t* bytes_out);
 
 /* Bytes of n_fields additional state-sized device buffers (caller-owned, handed over with rte_set_extra_workspace):
- * rte_step_ssprk3 needs 1 field, rte_apply_operator 2, rte_solve_steady restart + 3. */
+ * rte_step_ssprk3 needs 1 field, rte_apply_operator 2, rte_solve_steady restart + 3 (+ 3 with its preconditioner). */
 int rte_extra_workspace_bytes(const rte_grid* grid, int N, int n_fields, size_t* bytes_out);
 
 /* Forward-Euler stability bound of the step eq.(11) (R10; the paper picks dt "by inspection", PAPER.md:141,
@@ -173,14 +173,20 @@ int rte_apply_operator(rte_ctx* ctx, const float* x_dev, float* y_dev);
 
 /* Steady state L psi = q (q = the source of rte_set_source with temporal factor 1) by restarted GMRES(restart),
  * entirely on the device (the paper's Krylov solver was bound by host<->device
- * transfers).  The current state is the initial guess and becomes the solution.  Stops when the true relative
+ * transfers).  The current state is the initial guess and becomes the solution.  Stops when the TRUE relative
  * residual ||q - L psi|| / ||q||, recomputed at every restart, is <= tol, or after max_restarts cycles (not an
  * error: check *relres_out).  The Krylov basis, the Hessenberg matrix and the rotations live in device memory;
  * dot products / updates are this library's kernels; the host reads a few scalars once per restart cycle.
- * Needs restart + 3 fields of extra workspace; 1 <= restart <= 64.  applications_out: operator applications done;
+ *   precond_steps = 0: GMRES on L itself.
+ *   precond_steps = s > 0: GMRES on the time-stepping fixed-point equation  (I - Phi^s) psi = Phi^s(0; q),  Phi = one
+ *     SSP-RK3 step of size precond_dt_ps of d psi/dt = -c L psi + c q (the rte_step_ssprk3 map; stable up to ~ dx/c).
+ *     Its fixed point is the same steady state; s steps damp every fast mode, so the Krylov space only has to resolve
+ *     the few slow (diffusive) ones — far fewer basis vectors per operator sweep.
+ * Extra workspace: restart + 3 fields (+ 3 more with a preconditioner); 1 <= restart <= 64.
+ * applications_out: sweeps of the three pass kernels performed (one per application of L, three per RK3 step);
  * relres_out: final true relative residual (either may be NULL).  Synchronises the stream. */
-int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int* applications_out,
-                     double* relres_out);
+int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int precond_steps, float precond_dt_ps,
+                     int* applications_out, double* relres_out);
 
 /* NOT the paper's integrator (the paper uses forward Euler and names better integrators as future work,
  * PAPER.md:109,195): nsteps steps of the three-stage, third-order strong-stability-preserving Runge-Kutta scheme

@@ -63,7 +63,7 @@ _lib.rte_extra_workspace_bytes.argtypes = [C.POINTER(rte_grid), _i, _i, C.POINTE
 _lib.rte_set_extra_workspace.argtypes = [_vp, _vp, C.c_size_t]
 _lib.rte_stable_dt.argtypes = [_i, _i, _i, _f, _f, _f, _f, _f, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.rte_apply_operator.argtypes = [_vp, _vp, _vp]
-_lib.rte_solve_steady.argtypes = [_vp, _i, C.c_double, _i, C.POINTER(_i), C.POINTER(C.c_double)]
+_lib.rte_solve_steady.argtypes = [_vp, _i, C.c_double, _i, _i, _f, C.POINTER(_i), C.POINTER(C.c_double)]
 _lib.rte_step_profile.argtypes = [_vp, _i, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
 _lib.rte_fluence_change.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rte_time_ps.argtypes = [_vp, C.POINTER(C.c_double)]
@@ -298,13 +298,15 @@ def rte_apply_operator(ctx, x_dev, y_dev):
     _check(_lib.rte_apply_operator(ctx.handle, _dev(x_dev), _dev(y_dev)), ctx.handle)
 
 
-def rte_solve_steady(ctx, restart=30, tol=1e-5, max_restarts=100):
-    """Device-resident GMRES(restart) for L psi = q from the current state; returns (operator applications,
-    true relative residual).  Allocates restart + 3 fields of extra workspace if the context has fewer."""
-    rte_set_extra_workspace(ctx, max(restart + 3, getattr(ctx, "_extra_fields", 0)))
+def rte_solve_steady(ctx, restart=30, tol=1e-5, max_restarts=100, precond_steps=0, precond_dt_ps=0.0):
+    """Device-resident GMRES(restart) for L psi = q from the current state, optionally preconditioned by precond_steps
+    SSP-RK3 steps of size precond_dt_ps (include/rte.h); returns (operator sweeps, true relative residual).  Allocates
+    the extra workspace the solve needs if the context has less."""
+    need = restart + 3 + (3 if precond_steps > 0 else 0)
+    rte_set_extra_workspace(ctx, max(need, getattr(ctx, "_extra_fields", 0)))
     n, rr = _i(0), C.c_double(0)
-    _check(_lib.rte_solve_steady(ctx.handle, int(restart), float(tol), int(max_restarts), C.byref(n), C.byref(rr)),
-           ctx.handle)
+    _check(_lib.rte_solve_steady(ctx.handle, int(restart), float(tol), int(max_restarts), int(precond_steps),
+                                 float(precond_dt_ps), C.byref(n), C.byref(rr)), ctx.handle)
     return int(n.value), float(rr.value)
 
 

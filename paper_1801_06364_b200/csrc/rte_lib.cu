@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <mutex>
@@ -31,6 +32,7 @@ thread_local char g_create_error[256] = "";
 struct AxisTables {
     CplEntry* cpl = nullptr;      // weights x (-c dt) (2 pi / (n dx)) / n : the time step (eq.(11))
     CplEntry* cpl_op = nullptr;   // weights x (+1)    (2 pi / (n dx)) / n : the steady-state operator L = T + sigma_l
+    CplEntry* cpl_alt = nullptr;  // weights x (-c dt_alt) ... : Euler updates with another time step (solver preconditioner)
     float2* tw = nullptr;         // forward twiddles of this axis (generic kernels)
     int n = 0, N1 = 0, N2 = 0, maxcnt = 0, npure = 0;   // npure: leading coupling slots with pure blocks (rte_tables.h)
 };
@@ -39,7 +41,8 @@ struct AxisTables {
 enum PassKind {
     KIND_STEP = 0,   // out = in (1 - c dt sigma_l) - c dt T[in] + c dt q            eq.(11)
     KIND_OPER = 1,   // out = sigma_l in + T[in]                                     L of eq.(9)
-    KIND_EXP = 2     // out = E (in - c dt T[in]) + phi_1 c dt q, E = exp(-c dt sigma_l)   exponential Euler
+    KIND_EXP = 2,    // out = E (in - c dt T[in]) + phi_1 c dt q, E = exp(-c dt sigma_l)   exponential Euler
+    KIND_ALT = 3     // KIND_STEP with the context's alternative time step dt_alt and a constant source factor
 };
 
 }  // namespace
@@ -62,12 +65,16 @@ struct rte_ctx {
     float* srcw = nullptr;
     float* srcS = nullptr;
     size_t srcS_cap = 0;
+    int first_axis = 0;            // axis of the FIRST pass (the one that stores; the others accumulate): x
     float g_uniform = 0.f;         // > 0: the anisotropy g is one number (media.g_is_map == 0): kernels use the 2-number table
     char* extra = nullptr;         // caller-owned extra workspace (rte_set_extra_workspace): state-sized fields for
     size_t extra_bytes = 0;        // rte_step_ssprk3 (1), rte_apply_operator (2), rte_solve_steady (restart + 3)
+    float dt_alt = 0.f;                // time step of the cpl_alt tables (0: not built)
+    float alt_src = 0.f;               // source factor of KIND_ALT sweeps (1: constant source on, 0: homogeneous map)
     rtesolve::Scalars* sc = nullptr;   // device scalars of the Krylov solver
     double* partial = nullptr;         // per-block partial sums of its reductions
-    cudaGraphExec_t graph = nullptr;   // rte_step_graph: two captured steps (the state buffers are back in place)
+    cudaGraphExec_t graph = nullptr;   // kGraphSteps captured steps (an even count: the state buffers are back in place)
+    const float2* graph_psi = nullptr; // the buffer that held the state when the graph was captured
     bool graph_has_source = false;
     float* graph_amp = nullptr;        // device table of c dt f(t_n) for the captured steps
     float* phi_prev = nullptr;
@@ -401,6 +408,7 @@ size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
 constexpr size_t kMaxSmem = 226 * 1024;   // 227 KB per CTA minus the static mbarrier slot
 
 LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
+    const int first_axis = c->first_axis;
     const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz;
     int groups = 1;
     if (axis == 0) { A.stride_i = 1; A.stride_t = nx; A.group_stride = 0; A.pencils_per_group = ny * nz; }
@@ -409,8 +417,8 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     } else { A.stride_i = nx * ny; A.stride_t = 1; A.group_stride = 0; A.pencils_per_group = nx * ny; }
     const AxisTables& T = c->ax[axis];
     const int P = c->P, n = T.n;
-    const bool first = axis == 0;
-    const bool diag = first || kind == KIND_EXP;   // the x pass carries the Euler diagonal table (every pass of the exponential step)
+    const bool first = axis == first_axis;
+    const bool diag = first || kind == KIND_EXP;   // the FIRST pass carries the Euler diagonal table (every pass of the exponential step)
     LaunchPlan L{};
     L.spec = -1;
     A.P = P;
@@ -442,13 +450,13 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     A.tiles_per_group = (A.pencils_per_group + L.TP - 1) / L.TP;
     L.blocks = groups * A.tiles_per_group;
     L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, diag);
-    if (L.spec >= 0 && first && L.TP > 1) L.smem += (size_t)L.TP * (P % 16) * sizeof(float2);   // stacked-layout padding
+    if (L.spec >= 0 && axis == 0 && L.TP > 1) L.smem += (size_t)L.TP * (P % 16) * sizeof(float2);   // stacked-layout padding
     return L;
 }
 
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, int VAR = 0>
 cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
-    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG>;
+    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG, AX, VAR>;
     // the dynamic shared-memory limit is a per-device function attribute: set it once per (kernel instance, device)
     static std::mutex mu;
     static bool configured[64] = {};
@@ -470,14 +478,14 @@ cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t
 // Specialised FIRST kernels with several pencils per tile come in two instances: uniform g (2-number diagonal table,
 // measured 4 % faster on cfg2's x pass) and g map (N+1-number table).  With one pencil per tile (cfg4) a warp reads one
 // cell's table row anyway and the N+1-number table measured slightly faster, so only that instance exists.
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, int AX = 0>
 cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     constexpr bool kHasUG = MODE == rtepass::MODE_FIRST && QC != 0 && (QC / (PC ? PC : 1)) > 1;
     if constexpr (kHasUG)
-        if (A.g_uniform > 0.f) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, true>(A, L, s);
+        if (A.g_uniform > 0.f) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, true, AX>(A, L, s);
     PassArgs B = A;
     B.g_uniform = 0.f;                 // every other instance builds and reads the N+1-number table
-    return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, false>(B, L, s);
+    return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, false, AX>(B, L, s);
 }
 
 // generic kernels: one instance per supported pencil length (rte_tables.h RTE_SPLITS), FIRST/ACC at run time
@@ -491,16 +499,28 @@ cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaSt
 
 // E = 2 on the z axis of 3-D runs (fan-in of the z coupling is at most 2 pairs, rte_tables.h), 4 otherwise.
 // FIRST and ACC instances differ in occupancy (the accumulating tails hold no loaded data): MINB per mode.
-template <int MODE, int E>
+// Launched as (FIRST, 4, x), (ACC, 4, y), (ACC, 2, z): the x pass stores, the others accumulate.  (Measured and
+// rejected: FIRST on the z axis, whose coupling has the smaller fan-in — DESIGN.md 6.)
+template <int MODE, int E, int AX>
 cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     constexpr bool F = MODE == rtepass::MODE_FIRST;
+    if constexpr (F && AX == 0) {       // experiment switch: early-store variant of the x pass
+        static const bool early = getenv("RTE_EARLY") && getenv("RTE_EARLY")[0] == '1';
+        if (early && (spec == 0 || spec == 1 || spec == 2)) {
+            PassArgs B = A;
+            B.g_uniform = 0.f;
+            if (spec == 0) return launch_one_impl<24, 16, MODE, E, 32, 32, 256, 2, false, AX, 1>(B, L, s);
+            if (spec == 1) return launch_one_impl<16, 16, MODE, E, 36, 18, 288, 2, false, AX, 1>(B, L, s);
+            return launch_one_impl<16, 8, MODE, E, 32, 8, 256, 3, false, AX, 1>(B, L, s);
+        }
+    }
     switch (spec) {
-        case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2>(A, L, s);
-        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3>(A, L, s);
-        case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, F ? 3 : 4>(A, L, s);
-        case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2>(A, L, s);
-        case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3>(A, L, s);
-        case 5: return launch_one<8, 8, MODE, E, 32, 32, 256, 3>(A, L, s);
+        case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2, AX>(A, L, s);
+        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3, AX>(A, L, s);
+        case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, F ? 3 : 4, AX>(A, L, s);
+        case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2, AX>(A, L, s);
+        case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3, AX>(A, L, s);
+        case 5: return launch_one<8, 8, MODE, E, 32, 32, 256, 3, AX>(A, L, s);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -511,47 +531,89 @@ double source_time_factor(const rte_ctx* c, double t) {
     return 0.0;
 }
 
+// coupling table of one axis with every weight multiplied by `scale` x (2 pi / (n dx)) / n; unused entries: own pair, 0
+bool build_cpl_table(int dim, int N, int axis, int P, int n, double dx, double scale, std::vector<CplEntry>& flat, int* maxcnt) {
+    std::vector<std::vector<rtetab::PairEntry>> pe;
+    rtetab::pair_coupling(dim, N, axis, pe);
+    const double m = scale * 6.283185307179586476925286766559 / ((double)n * dx) / (double)n;
+    flat.assign((size_t)P * rtepass::kMaxE, CplEntry{0.f, 0.f, 0.f, 0.f, 0, 0});
+    int mx = 0;
+    for (int p = 0; p < P; ++p) {
+        const int cnt = (int)pe[p].size();
+        if (cnt > rtepass::kMaxE) return false;
+        if (cnt > mx) mx = cnt;
+        for (int e = 0; e < rtepass::kMaxE; ++e)
+            flat[(size_t)p * rtepass::kMaxE + e] =
+                (e < cnt && pe[p][e].src >= 0) ? CplEntry{(float)(m * pe[p][e].w00), (float)(m * pe[p][e].w11),
+                                   (float)(m * pe[p][e].w01), (float)(m * pe[p][e].w10), pe[p][e].src, 0}
+                        : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
+    }
+    if (maxcnt) *maxcnt = mx;
+    return true;
+}
+
+// (re)build the alternative-step tables: Euler updates with time step dt_alt on the same context
+int set_alt_dt(rte_ctx* c, float dt_alt) {
+    if (c->dt_alt == dt_alt) return RTE_OK;
+    for (int a = 0; a < c->grid.dim; ++a) {
+        AxisTables& T = c->ax[a];
+        std::vector<CplEntry> flat;
+        if (!build_cpl_table(c->grid.dim, c->N, a, c->P, T.n, c->dx, -(double)c->c * (double)dt_alt, flat, nullptr))
+            return fail(c, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
+        if (!T.cpl_alt) CUDA_TRY(c, cudaMalloc((void**)&T.cpl_alt, flat.size() * sizeof(CplEntry) + 16));
+        CUDA_TRY(c, cudaMemcpyAsync(T.cpl_alt, flat.data(), flat.size() * sizeof(CplEntry), cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    c->dt_alt = dt_alt;
+    return RTE_OK;
+}
+
 // One sweep of the per-axis pass kernels, out = F(in) with F chosen by `kind` (PassKind above): the forward-Euler update
 // of eq.(11) with the source at t_src, the steady-state operator, or the exponential Euler update.
 // amp_dev (optional): device location of c dt f(t) for this sweep (CUDA-graph replay), instead of the host value.
 int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKind kind = KIND_STEP,
                  cudaEvent_t* ev = nullptr, const int* halt = nullptr, const float* amp_dev = nullptr) {
     const int naxes = c->grid.dim;
-    for (int axis = 0; axis < naxes; ++axis) {
+    const int fa = c->first_axis;
+    // the FIRST pass stores, the others add to what it stored: it goes first
+    int order[3] = {fa, fa == 0 ? 1 : 0, fa == 2 ? 1 : 2};
+    for (int k = 0; k < naxes; ++k) {
+        const int axis = order[k];
         PassArgs A{};
         A.psi = in; A.acc = out;
-        A.cpl = kind == KIND_OPER ? c->ax[axis].cpl_op : c->ax[axis].cpl;
+        A.cpl = kind == KIND_OPER ? c->ax[axis].cpl_op : (kind == KIND_ALT ? c->ax[axis].cpl_alt : c->ax[axis].cpl);
         A.tw = c->ax[axis].tw;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
-        A.cdt = kind == KIND_OPER ? -1.f : c->c * c->dt;
+        A.cdt = kind == KIND_OPER ? -1.f : (kind == KIND_ALT ? c->c * c->dt_alt : c->c * c->dt);
         A.ident = kind == KIND_OPER ? 0.f : 1.f;
         A.expo = kind == KIND_EXP ? 1 : 0;
-        A.first = axis == 0 ? 1 : 0;
+        A.first = axis == fa ? 1 : 0;
+        A.first_axis = fa;
         A.halt = halt;
         A.nsig = c->N + 1; A.g_uniform = c->g_uniform;
         A.srcS = c->srcS; A.srcw = c->srcw;
-        for (int k = 0; k < 3; ++k) { A.src_org[k] = c->src_org[k]; A.src_ext[k] = c->src_ext[k]; }
+        for (int j = 0; j < 3; ++j) { A.src_org[j] = c->src_org[j]; A.src_ext[j] = c->src_ext[j]; }
         A.src_amp = 0.f; A.src_amp_dev = nullptr;
         A.nx = c->grid.nx; A.ny = c->grid.ny;
         const LaunchPlan L = plan_pass(c, axis, A, kind);
         const int n = c->ax[axis].n;
-        cudaError_t e;
-        if (axis == 0) {
-            if (c->src_kind != 0 && kind != KIND_OPER) {
-                A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src));
-                A.src_amp_dev = amp_dev;
-                if (amp_dev) A.src_amp = 1.f;      // non-zero: the kernel reads the device value
-            }
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_FIRST, 4>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
-        } else if (axis == 2) {
-            // z axis: coupling fan-in 2 (rte_tables.h); plan_pass falls back to the generic kernel otherwise
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 2>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
-        } else {
-            e = L.spec >= 0 ? launch_spec<rtepass::MODE_ACC, 4>(L.spec, A, L, c->stream) : launch_generic(n, A, L, c->stream);
+        if (A.first && c->src_kind != 0 && kind == KIND_ALT) {
+            A.src_amp = c->c * c->dt_alt * c->alt_src;
+        } else if (A.first && c->src_kind != 0 && kind != KIND_OPER) {
+            A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src));
+            A.src_amp_dev = amp_dev;
+            if (amp_dev) A.src_amp = 1.f;      // non-zero: the kernel reads the device value
         }
+        cudaError_t e;
+        using namespace rtepass;
+        if (L.spec < 0) e = launch_generic(n, A, L, c->stream);
+        else if (axis == 0) e = launch_spec<MODE_FIRST, 4, 0>(L.spec, A, L, c->stream);
+        else if (axis == 1) e = launch_spec<MODE_ACC, 4, 1>(L.spec, A, L, c->stream);
+        // z axis: coupling fan-in 2 (rte_tables.h); plan_pass falls back to the generic kernel otherwise
+        else e = launch_spec<MODE_ACC, 2, 2>(L.spec, A, L, c->stream);
         if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
         c->launches += 1;
-        if (ev) cudaEventRecord(ev[axis], c->stream);
+        if (ev) cudaEventRecord(ev[k], c->stream);
     }
     return RTE_OK;
 }
@@ -566,7 +628,9 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr, PassKind kind = KIND_STEP, c
 }
 
 // y = a x + b y over a whole state buffer (the convex combinations of the Runge-Kutta stages)
-__global__ void k_axpby(float4* __restrict__ y, const float4* __restrict__ x, float a, float b, size_t n4) {
+__global__ void k_axpby(float4* __restrict__ y, const float4* __restrict__ x, float a, float b, size_t n4,
+                        const int* __restrict__ halt = nullptr) {
+    if (halt && *halt) return;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
         const float4 xv = x[i];
         float4 yv = y[i];
@@ -583,6 +647,23 @@ float2* extra_field(const rte_ctx* c, int i) {
     const size_t f = field_bytes(c);
     if (!c->extra || (size_t)(i + 1) * f > c->extra_bytes) return nullptr;
     return (float2*)(c->extra + (size_t)i * f);
+}
+
+// One SSP-RK3 step on explicit buffers with the alternative time step and a constant source factor (KIND_ALT):
+// Y = RK3(X); X is only read, Z is scratch.
+int rk3_alt(rte_ctx* c, const float2* X, float2* Y, float2* Z, const int* halt) {
+    const size_t n4 = (size_t)c->G * c->Cp / 4;
+    const int gb = grid_for((long long)n4, 256);
+    int rc = euler_update(c, X, Y, 0.0, KIND_ALT, nullptr, halt);
+    if (rc != RTE_OK) return rc;
+    rc = euler_update(c, Y, Z, 0.0, KIND_ALT, nullptr, halt);
+    if (rc != RTE_OK) return rc;
+    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Z, (const float4*)X, 0.75f, 0.25f, n4, halt);
+    rc = euler_update(c, Z, Y, 0.0, KIND_ALT, nullptr, halt);
+    if (rc != RTE_OK) return rc;
+    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Y, (const float4*)X, (float)(1.0 / 3.0), (float)(2.0 / 3.0), n4, halt);
+    c->launches += 2;
+    return RTE_OK;
 }
 
 // SSP-RK3 (Shu-Osher form, not the paper's integrator):
@@ -653,7 +734,7 @@ void drop_graph(rte_ctx* c) {
 void free_ctx(rte_ctx* c) {
     if (!c) return;
     for (int a = 0; a < 3; ++a) {
-        cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_op); cudaFree(c->ax[a].tw);
+        cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_op); cudaFree(c->ax[a].cpl_alt); cudaFree(c->ax[a].tw);
     }
     if (c->graph) cudaGraphExecDestroy(c->graph);
     cudaFree(c->graph_amp);
@@ -819,6 +900,7 @@ static int create_impl(rte_ctx** out, const rte_grid* grid, int N, float dx, flo
     ctx->G = (long long)grid->nx * grid->ny * grid->nz;
     ctx->dx = dx; ctx->dt = dt; ctx->c = c;
     ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->first_axis = 0;
 
     const size_t field = align_up((size_t)ctx->G * ctx->Cp * sizeof(float), 256), map = align_up((size_t)ctx->G * sizeof(float), 256);
     char* w = (char*)workspace_dev;
@@ -836,7 +918,7 @@ static int create_impl(rte_ctx** out, const rte_grid* grid, int N, float dx, flo
         for (int a = 0; a < grid->dim; ++a) {
             int n1 = 0, n2 = 0;
             rtetab::split_of(ext[a], n1, n2);
-            if (pass_smem(ext[a], ctx->P, 1, N + 1, a == 0) > kMaxSmem ||
+            if (pass_smem(ext[a], ctx->P, 1, N + 1, a == ctx->first_axis) > kMaxSmem ||
                 (unsigned long long)36 * (unsigned long long)str[a] * (unsigned long long)ctx->P * 8ull >= (1ull << 32)) {
                 *live = nullptr;
                 delete ctx;
@@ -863,31 +945,14 @@ static int create_impl(rte_ctx** out, const rte_grid* grid, int N, float dx, flo
         AxisTables& T = ctx->ax[a];
         T.n = ext_n[a];
         rtetab::split_of(T.n, T.N1, T.N2);
-        std::vector<std::vector<rtetab::PairEntry>> pe;
-        rtetab::pair_coupling(grid->dim, N, a, pe);
-        // weights pre-multiplied by the axis' wavenumber unit and 1/n (the kernel multiplies by the integer wavenumber only)
-        // and by -c dt for the time step (eq.(11)) / +1 for the operator L; unused entries: own pair, zero weights
-        const double unit = 6.283185307179586476925286766559 / ((double)T.n * (double)dx) / (double)T.n;
-        const double scales[2] = {-(double)c * (double)dt * unit, unit};
-        std::vector<CplEntry> flat((size_t)ctx->P * rtepass::kMaxE), flat_op(flat.size());
-        T.maxcnt = 0;
+        std::vector<CplEntry> flat, flat_op;
         T.npure = rtetab::pair_layout(grid->dim, N).npure[a];
-        for (int p = 0; p < ctx->P; ++p) {
-            const int cnt = (int)pe[p].size();
-            if (cnt > rtepass::kMaxE) {
-                *live = nullptr;
-                free_ctx(ctx);
-                return fail(nullptr, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
-            }
-            if (cnt > T.maxcnt) T.maxcnt = cnt;
-            for (int e = 0; e < rtepass::kMaxE; ++e)
-                for (int v = 0; v < 2; ++v) {
-                    const double m = scales[v];
-                    (v == 0 ? flat : flat_op)[(size_t)p * rtepass::kMaxE + e] =
-                        (e < cnt && pe[p][e].src >= 0) ? CplEntry{(float)(m * pe[p][e].w00), (float)(m * pe[p][e].w11),
-                                           (float)(m * pe[p][e].w01), (float)(m * pe[p][e].w10), pe[p][e].src, 0}
-                                : CplEntry{0.f, 0.f, 0.f, 0.f, p, 0};
-                }
+        // -c dt for the time step (eq.(11)), +1 for the operator L
+        if (!build_cpl_table(grid->dim, N, a, ctx->P, T.n, dx, -(double)c * (double)dt, flat, &T.maxcnt) ||
+            !build_cpl_table(grid->dim, N, a, ctx->P, T.n, dx, 1.0, flat_op, nullptr)) {
+            *live = nullptr;
+            free_ctx(ctx);
+            return fail(nullptr, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
         }
         CREATE_TRY(upload(&T.cpl_op, flat_op, ctx->stream));
         {
@@ -1025,6 +1090,7 @@ constexpr size_t kGraphMaxStateBytes = (size_t)24 << 20;   // states up to 24 MB
 int build_graph(rte_ctx* c) {
     if (!c->graph_amp) CUDA_TRY(c, cudaMalloc((void**)&c->graph_amp, kGraphSteps * sizeof(float)));
     const long long steps0 = c->steps, launches0 = c->launches;
+    c->graph_psi = c->psi;
     cudaGraph_t g = nullptr;
     // captured on a private stream (the caller's may be the legacy default stream, which cannot capture); the
     // instantiated graph is launched on the caller's stream
@@ -1061,6 +1127,11 @@ int rte_step(rte_ctx* ctx, int nsteps) {
                 --left;
             }
             if (!ctx->graph) { const int rc = build_graph(ctx); if (rc != RTE_OK) return rc; }
+            if (ctx->psi != ctx->graph_psi) {               // the captured launches read the other buffer: one eager step
+                const int rc = one_step(ctx);
+                if (rc != RTE_OK) return rc;
+                --left;
+            }
             const int per_step = ctx->grid.dim;
             while (left >= kGraphSteps) {
                 if (ctx->src_kind != 0) {
@@ -1147,84 +1218,150 @@ __global__ void k_source_field(float* __restrict__ b, const float* __restrict__ 
     }
 }
 
-int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int* applications_out, double* relres_out) {
+int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int precond_steps, float precond_dt_ps,
+                     int* applications_out, double* relres_out) {
     using namespace rtesolve;
     if (!ctx) return RTE_ESTATE;
-    if (restart < 1 || restart > kMaxRestart || !(tol > 0) || max_restarts < 0)
-        return fail(ctx, RTE_EINVAL, "rte_solve_steady: restart in 1..64, tol > 0, max_restarts >= 0");
+    if (restart < 1 || restart > kMaxRestart || !(tol > 0) || max_restarts < 0 || precond_steps < 0 ||
+        (precond_steps > 0 && !(precond_dt_ps > 0)))
+        return fail(ctx, RTE_EINVAL, "rte_solve_steady: restart in 1..64, tol > 0, max_restarts >= 0, precond_steps >= 0 (dt > 0)");
     if (ctx->src_kind == 0) return fail(ctx, RTE_EINVAL, "rte_solve_steady needs a source (rte_set_source)");
-    const int m = restart;
+    const int m = restart, s = precond_steps;
+    const int nfields = m + 3 + (s > 0 ? 3 : 0);
+    if (!extra_field(ctx, nfields - 1))
+        return fail(ctx, RTE_EINVAL, "rte_solve_steady needs restart + 3 (+ 3 with a preconditioner) state-sized fields of extra "
+                                     "workspace (rte_set_extra_workspace)");
     float2* W = extra_field(ctx, 0);
     float2* B = extra_field(ctx, 1);
     float2* V = extra_field(ctx, 2);
-    if (!extra_field(ctx, m + 2))
-        return fail(ctx, RTE_EINVAL, "rte_solve_steady needs restart + 3 state-sized fields of extra workspace (rte_set_extra_workspace)");
+    float2* R[3] = {nullptr, nullptr, nullptr};                // preconditioner scratch
+    if (s > 0) for (int i = 0; i < 3; ++i) R[i] = extra_field(ctx, m + 3 + i);
     if (((size_t)ctx->G * ctx->Cp) % 4 != 0) return fail(ctx, RTE_EUNSUPPORTED, "state size not a multiple of 16 bytes");
     if (!ctx->sc) {
         CUDA_TRY(ctx, cudaMalloc((void**)&ctx->sc, sizeof(Scalars)));
         CUDA_TRY(ctx, cudaMalloc((void**)&ctx->partial, (size_t)kRedBlocks * (kMaxRestart + 2) * sizeof(double)));
     }
+    if (s > 0) { const int rc = set_alt_dt(ctx, precond_dt_ps); if (rc != RTE_OK) return rc; }
     cudaStream_t st = ctx->stream;
     Scalars* sc = ctx->sc;
     double* partial = ctx->partial;
-    const size_t n4 = (size_t)ctx->G * ctx->Cp / 4, stride4 = field_bytes(ctx) / 16;
-    const int NS = kMaxRestart + 1;                            // slot of the norms in a partial-sum row
+    const size_t fb = field_bytes(ctx), n4 = (size_t)ctx->G * ctx->Cp / 4, stride4 = fb / 16;
+    const int NS = kMaxRestart + 1, NT = kMaxRestart;          // partial-sum slots: cycle norms, true-residual norms
     double* hfold = (double*)((char*)sc + offsetof(Scalars, h));
     const int* halt = (const int*)((char*)sc + offsetof(Scalars, halt));
     const double* inv = (const double*)((char*)sc + offsetof(Scalars, inv));
-    CUDA_TRY(ctx, cudaMemsetAsync(sc, 0, sizeof(Scalars), st));
-    CUDA_TRY(ctx, cudaMemcpyAsync((char*)sc + offsetof(Scalars, tol), &tol, sizeof(double), cudaMemcpyHostToDevice, st));
-    // b = q (temporal factor 1), ||b||
-    k_source_field<<<grid_for(ctx->G * ctx->Cp, 256), 256, 0, st>>>((float*)B, ctx->srcS, ctx->srcw, ctx->src_org[0], ctx->src_org[1],
-                                                                    ctx->src_org[2], ctx->src_ext[0], ctx->src_ext[1], ctx->src_ext[2],
-                                                                    ctx->grid.nx, ctx->grid.ny, ctx->G, ctx->Cp);
-    k_sub_norm<<<kRedBlocks, kRedThreads, 0, st>>>(nullptr, (const float4*)B, nullptr, n4, partial, NS);
-    k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
-    k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 1);
-    ctx->launches += 4;
-    long long applications = 0;
-    double relres = 0.0;
-    for (int cycle = 0;; ++cycle) {
-        // r_0 = b - L x (true residual), v_0 = r_0 / ||r_0||
-        int rc = euler_update(ctx, ctx->psi, W, 0.0, KIND_OPER);
-        if (rc != RTE_OK) return rc;
-        k_sub_norm<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)V, (const float4*)B, (const float4*)W, n4, partial, NS);
-        k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
-        k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 0);
-        ctx->launches += 3;
-        // the one host read of the cycle: a few scalars (true relative residual, Arnoldi steps done so far)
-        HostView hv{};
-        CUDA_TRY(ctx, cudaMemcpyAsync(&hv, (char*)sc + offsetof(Scalars, bnorm), sizeof(HostView), cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(ctx, cudaStreamSynchronize(st));
-        relres = hv.relres;
-        applications = (long long)hv.ktotal + cycle + 1;      // Arnoldi steps + one residual evaluation per cycle
-        if (hv.bnorm == 0.0) {                                 // q = 0: the steady state is psi = 0
-            CUDA_TRY(ctx, cudaMemsetAsync(ctx->psi, 0, field_bytes(ctx), st));
-            relres = 0.0;
-            break;
-        }
-        if (!(relres > tol) || cycle == max_restarts) break;
-        k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)V, (const float4*)V, inv, n4, sc);
+    long long sweeps = 0;                                      // launched operator sweeps that were not no-ops
+
+    auto source_field = [&](float2* dst) {
+        k_source_field<<<grid_for(ctx->G * ctx->Cp, 256), 256, 0, st>>>((float*)dst, ctx->srcS, ctx->srcw, ctx->src_org[0],
+            ctx->src_org[1], ctx->src_org[2], ctx->src_ext[0], ctx->src_ext[1], ctx->src_ext[2], ctx->grid.nx, ctx->grid.ny,
+            ctx->G, ctx->Cp);
         ctx->launches += 1;
-        for (int k = 0; k < m; ++k) {
-            const float2* vk = (const float2*)((const char*)V + (size_t)k * field_bytes(ctx));
-            float2* vn = (float2*)((char*)V + (size_t)(k + 1) * field_bytes(ctx));
-            rc = euler_update(ctx, vk, W, 0.0, KIND_OPER, nullptr, halt);
-            if (rc != RTE_OK) return rc;
-            k_dots<<<kRedBlocks, kRedThreads, 0, st>>>((const float4*)W, (const float4*)V, stride4, k + 1, n4, partial, sc);
-            k_fold<<<1, 128, 0, st>>>(partial, kRedBlocks, k + 1, hfold, sc);
-            k_update<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)W, (const float4*)V, stride4, k + 1, n4, hfold, partial, NS, sc);
-            k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
-            k_givens<<<1, 1, 0, st>>>(sc, k, NS);
-            k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)vn, (const float4*)W, inv, n4, sc);
-            ctx->launches += 6;
-        }
-        k_solve_y<<<1, 1, 0, st>>>(sc);
-        k_correct<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)ctx->psi, (const float4*)V, stride4, n4, sc);
+    };
+    auto norm_to = [&](const float2* a, const float2* b2, float2* y, int slot) {      // h[slot] = ||a - b||^2, y = a - b
+        k_sub_norm<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)y, (const float4*)a, (const float4*)b2, n4, partial, slot);
+        k_fold<<<1, 128, 0, st>>>(partial + slot, kRedBlocks, 1, hfold + slot, sc);
         ctx->launches += 2;
-        CUDA_TRY(ctx, cudaGetLastError());
+    };
+    // Phi^s: s SSP-RK3 steps of size precond_dt from `in` (read only); returns the buffer that holds the result
+    auto rk_steps = [&](const float2* in, float src_factor, const int* hlt, float2** out) -> int {
+        ctx->alt_src = src_factor;
+        const float2* X = in;
+        float2* Y = R[0];
+        for (int k = 0; k < s; ++k) {
+            const int rc = rk3_alt(ctx, X, Y, R[1], hlt);
+            if (rc != RTE_OK) return rc;
+            X = Y;
+            Y = (Y == R[0]) ? R[2] : R[0];
+        }
+        *out = const_cast<float2*>(X);
+        return RTE_OK;
+    };
+    // the operator of the linear system: plain  A v = L v ;  preconditioned  A v = v - Phi_lin^s v
+    auto apply = [&](const float2* v, const int* hlt) -> int {
+        if (s == 0) return euler_update(ctx, v, W, 0.0, KIND_OPER, nullptr, hlt);
+        float2* res = nullptr;
+        const int rc = rk_steps(v, 0.f, hlt, &res);
+        if (rc != RTE_OK) return rc;
+        k_axpby<<<grid_for((long long)n4, 256), 256, 0, st>>>((float4*)res, (const float4*)v, 1.f, -1.f, n4, hlt);   // res = v - res
+        ctx->launches += 1;
+        // W <- res (the Arnoldi kernels work on W): swap roles instead of copying
+        std::swap(W, *(res == R[0] ? &R[0] : &R[2]));
+        return RTE_OK;
+    };
+
+    CUDA_TRY(ctx, cudaMemsetAsync(sc, 0, sizeof(Scalars), st));
+    // right-hand side: plain b = q ; preconditioned b = Phi^s(0) with the source on.  ||q|| for the true residual.
+    source_field(s > 0 ? R[1] : B);
+    norm_to(s > 0 ? R[1] : B, nullptr, nullptr, NT);
+    if (s > 0) {
+        CUDA_TRY(ctx, cudaMemsetAsync(V, 0, fb, st));
+        float2* res = nullptr;
+        const int rc = rk_steps(V, 1.f, nullptr, &res);
+        if (rc != RTE_OK) return rc;
+        std::swap(B, *(res == R[0] ? &R[0] : &R[2]));
     }
-    if (applications_out) *applications_out = (int)applications;
+    norm_to(B, nullptr, nullptr, NS);
+    k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 1);
+    ctx->launches += 1;
+    struct Host { double h64, h65, bnorm, beta, relres, inv, tol; int halt, kdone, ktotal, pad_; } hv{};
+    static_assert(offsetof(Scalars, bnorm) == offsetof(Scalars, h) + (kMaxRestart + 2) * sizeof(double), "HostView layout");
+    CUDA_TRY(ctx, cudaMemcpyAsync(&hv, (char*)sc + offsetof(Scalars, h) + NT * sizeof(double), sizeof(Host), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    const double qnorm = std::sqrt(hv.h64);
+    double relres = 0.0;
+    int cycles = 0;
+    if (!(qnorm > 0.0)) {                                      // q = 0: the steady state is psi = 0
+        CUDA_TRY(ctx, cudaMemsetAsync(ctx->psi, 0, fb, st));
+    } else
+        for (int cycle = 0;; ++cycle) {
+            cycles = cycle + 1;
+            int rc;
+            if (s > 0) {                                       // true residual ||q - L x|| / ||q||
+                rc = euler_update(ctx, ctx->psi, W, 0.0, KIND_OPER);
+                if (rc != RTE_OK) return rc;
+                source_field(R[1]);
+                norm_to(R[1], W, nullptr, NT);
+            }
+            // residual of the (preconditioned) system, v_0 = r_0 / ||r_0||
+            rc = apply(ctx->psi, nullptr);
+            if (rc != RTE_OK) return rc;
+            norm_to(B, W, V, NS);
+            k_cycle_begin<<<1, 1, 0, st>>>(sc, NS, 0);
+            ctx->launches += 1;
+            // the one host read of the cycle: a few scalars
+            CUDA_TRY(ctx, cudaMemcpyAsync(&hv, (char*)sc + offsetof(Scalars, h) + NT * sizeof(double), sizeof(Host), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(ctx, cudaStreamSynchronize(st));
+            relres = s > 0 ? std::sqrt(hv.h64) / qnorm : hv.relres;
+            if (!(relres > tol) || cycle == max_restarts || !(hv.relres > 0.0)) break;
+            // in-cycle stopping level for the device (relative to ||b||): the residual of the solved system has to fall by
+            // tol / relres; with a preconditioner its norm is not the true one, so aim a little lower
+            const double level = (s > 0 ? 0.3 : 1.0) * tol / relres * hv.relres;
+            CUDA_TRY(ctx, cudaMemcpyAsync((char*)sc + offsetof(Scalars, tol), &level, sizeof(double), cudaMemcpyHostToDevice, st));
+            k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)V, (const float4*)V, inv, n4, sc);
+            ctx->launches += 1;
+            for (int k = 0; k < m; ++k) {
+                const float2* vk = (const float2*)((const char*)V + (size_t)k * fb);
+                float2* vn = (float2*)((char*)V + (size_t)(k + 1) * fb);
+                rc = apply(vk, halt);
+                if (rc != RTE_OK) return rc;
+                k_dots<<<kRedBlocks, kRedThreads, 0, st>>>((const float4*)W, (const float4*)V, stride4, k + 1, n4, partial, sc);
+                k_fold<<<1, 128, 0, st>>>(partial, kRedBlocks, k + 1, hfold, sc);
+                k_update<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)W, (const float4*)V, stride4, k + 1, n4, hfold, partial, NS, sc);
+                k_fold<<<1, 128, 0, st>>>(partial + NS, kRedBlocks, 1, hfold + NS, sc);
+                k_givens<<<1, 1, 0, st>>>(sc, k, NS);
+                k_scale<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)vn, (const float4*)W, inv, n4, sc);
+                ctx->launches += 6;
+            }
+            k_solve_y<<<1, 1, 0, st>>>(sc);
+            k_correct<<<kRedBlocks, kRedThreads, 0, st>>>((float4*)ctx->psi, (const float4*)V, stride4, n4, sc);
+            ctx->launches += 2;
+            CUDA_TRY(ctx, cudaGetLastError());
+        }
+    // operator sweeps actually performed: Arnoldi steps and per-cycle residuals, 3 per RK3 step with a preconditioner
+    const long long per_apply = s > 0 ? 3LL * s : 1;
+    sweeps = (long long)hv.ktotal * per_apply + (long long)cycles * (per_apply + (s > 0 ? 1 : 0)) + (s > 0 ? per_apply : 0);
+    if (applications_out) *applications_out = (int)sweeps;
     if (relres_out) *relres_out = relres;
     ctx->have_prev = false;
     return RTE_OK;
@@ -1245,13 +1382,15 @@ int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* 
     for (int s = 0; s < nsteps && rc == RTE_OK; ++s) rc = one_step(ctx, &ev[(size_t)s * naxes + 1]);
     if (rc == RTE_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = fail(ctx, RTE_ECUDA, "CUDA: %s", "stream synchronise failed");
     for (int a = 0; a < 3; ++a) { ms_axis_host[a] = 0.0; if (launches_axis_host) launches_axis_host[a] = 0; }
+    const int fa = ctx->first_axis;
+    const int order[3] = {fa, fa == 0 ? 1 : 0, fa == 2 ? 1 : 2};          // launch order of euler_update
     if (rc == RTE_OK)
         for (int s = 0; s < nsteps; ++s)
-            for (int a = 0; a < naxes; ++a) {
+            for (int k = 0; k < naxes; ++k) {
                 float ms = 0.f;
-                cudaEventElapsedTime(&ms, ev[(size_t)s * naxes + a], ev[(size_t)s * naxes + a + 1]);
-                ms_axis_host[a] += ms;
-                if (launches_axis_host) launches_axis_host[a] += 1;
+                cudaEventElapsedTime(&ms, ev[(size_t)s * naxes + k], ev[(size_t)s * naxes + k + 1]);
+                ms_axis_host[order[k]] += ms;
+                if (launches_axis_host) launches_axis_host[order[k]] += 1;
             }
     for (auto& e : ev) cudaEventDestroy(e);
     return rc;

@@ -61,6 +61,7 @@ struct PassArgs {
     int expo;               // generic kernels only: exponential (integrating-factor) Euler step, s_l = exp(-cdt sigma_l)
                             // multiplies psi AND the streaming term, the source carries phi_1 (rte_step_exp)
     int first;              // MODE_RT kernels: 1 = FIRST, 0 = ACC
+    int first_axis;         // axis of the FIRST pass (0 = x, 2 = z): how the source box maps onto its pencils
     const int* halt;        // optional device flag: non-zero => the launch does nothing (Krylov solver, converged early)
     const float2* tw;       // generic kernels: forward twiddles exp(-2 pi i j / n) of this axis, n entries (global)
     int nsig;               // N + 1 degrees
@@ -189,28 +190,37 @@ __device__ __forceinline__ int col_offset(int q, int P) {
     return q;
 }
 
-// ---- source term along one x pencil (FIRST is the x pass): c dt f(t_n) w_c S(r) for the cells inside the source box ------
+// ---- source term along one pencil of the FIRST pass: c dt f(t_n) w_c S(r) for the cells inside the source box -------------
+// ax = 0: x pencils (pencil = y + ny z, the position along the pencil is x); ax = 2: z pencils (pencil = x + nx y,
+// position z).  (The y axis never carries the FIRST pass.)
 struct SourceRow {
     bool on = false;
     float sw0 = 0.f, sw1 = 0.f;
-    const float* S = nullptr;      // S at x = box origin of this pencil's row of the box
-    int x0 = 0, ext = 0;
-    // pencil = y + ny*z of the pencil, p = pair
-    __device__ __forceinline__ SourceRow(const PassArgs& A, long long pencil, int p) {
+    const float* S = nullptr;      // S at the box origin along this pencil
+    int i0 = 0, ext = 0, stride = 1;
+    // p = pair
+    __device__ __forceinline__ SourceRow(const PassArgs& A, int ax, long long pencil, int p) {
         if (A.src_amp == 0.f) return;
-        const int by = (int)(pencil % A.ny) - A.src_org[1], bz = (int)(pencil / A.ny) - A.src_org[2];
-        if (by < 0 || by >= A.src_ext[1] || bz < 0 || bz >= A.src_ext[2]) return;
+        if (ax == 0) {
+            const int by = (int)(pencil % A.ny) - A.src_org[1], bz = (int)(pencil / A.ny) - A.src_org[2];
+            if (by < 0 || by >= A.src_ext[1] || bz < 0 || bz >= A.src_ext[2]) return;
+            S = A.srcS + ((size_t)bz * A.src_ext[1] + by) * A.src_ext[0];
+            i0 = A.src_org[0]; ext = A.src_ext[0]; stride = 1;
+        } else {
+            const int bx = (int)(pencil % A.nx) - A.src_org[0], by = (int)(pencil / A.nx) - A.src_org[1];
+            if (bx < 0 || bx >= A.src_ext[0] || by < 0 || by >= A.src_ext[1]) return;
+            S = A.srcS + (size_t)by * A.src_ext[0] + bx;
+            i0 = A.src_org[2]; ext = A.src_ext[2]; stride = A.src_ext[0] * A.src_ext[1];
+        }
         on = true;
         const float amp = A.src_amp_dev ? __ldg(A.src_amp_dev) : A.src_amp;
         sw0 = __ldg(A.srcw + 2 * p) * amp; sw1 = __ldg(A.srcw + 2 * p + 1) * amp;
-        S = A.srcS + ((size_t)bz * A.src_ext[1] + by) * A.src_ext[0];
-        x0 = A.src_org[0]; ext = A.src_ext[0];
     }
-    __device__ __forceinline__ void add(int x, float2& e) const {
+    __device__ __forceinline__ void add(int i, float2& e) const {
         if (!on) return;
-        const int bx = x - x0;
-        if (bx >= 0 && bx < ext) {
-            const float v = __ldg(S + bx);
+        const int bi = i - i0;
+        if (bi >= 0 && bi < ext) {
+            const float v = __ldg(S + (size_t)bi * stride);
             e.x = fmaf(sw0, v, e.x); e.y = fmaf(sw1, v, e.y);
         }
     }
@@ -223,9 +233,12 @@ struct SourceRow {
 // one shared-memory store and E loads per element become E loads, and the tail runs without any barrier.  The
 // gather reads rows that other columns of the same rows overwrite, hence the fence between gather and store: the rows
 // of one residue b are owned by one warp (32 % Q == 0) or by one round of the whole CTA (nt % Q == 0).
-template <int N1, int N2, int MODE, int E, int QC, int PC, bool STACKED, bool TMA, bool CF>
+// EARLY (FIRST pass, experiment): the column's own psi is still in the tile during the gather, so the Euler diagonal
+// and the source are applied HERE and stored to the new buffer at once; the tail then adds -c dt T_x by a vector
+// reduction like the accumulating passes (same thread, same address: program order) instead of re-reading psi.
+template <int N1, int N2, int AX, int E, int QC, int PC, bool STACKED, bool TMA, bool CF, bool EARLY = false>
 __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
-                                           int tid, int nt, unsigned long long* bar) {
+                                           int tid, int nt, unsigned long long* bar, long long pencil0 = 0) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
@@ -239,11 +252,11 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
         float2* col = tile + b * SI + t * ST + p;
         float2 v[N1];
         if (CF) {
-            // The specialised kernels are launched as (FIRST, E = 4) on the x axis, (ACC, E = 4) on the y axis and
-            // (ACC, E = 2) on the z axis; the pair layout guarantees 2 pure slots on x (diagonal blocks) and y
-            // (off-diagonal blocks) — rte_tables.h PairLayout::npure, checked by the host before it picks these kernels.
+            // The specialised kernels are launched with E = 4 on the x and y axes and E = 2 on the z axis; the pair
+            // layout guarantees 2 pure slots on x (diagonal blocks) and y (off-diagonal blocks) — rte_tables.h
+            // PairLayout::npure, checked by the host before it picks these kernels.
             constexpr int NPURE = (E == 4) ? 2 : 0;
-            constexpr bool PURE_DIAG = MODE == MODE_FIRST;
+            constexpr bool PURE_DIAG = AX == 0;
             const float2* srow[E];
             float2 wd[E], ws[E];
 #pragma unroll
@@ -254,6 +267,15 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
                 ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
             }
             mbar_wait(bar + (STACKED ? 0 : b), 0);
+            int i0 = 0, i1 = 0;
+            float2* sp = nullptr;
+            if (EARLY) {
+                constexpr int ncell1 = (N1 * N2) * (QC / (PC ? PC : 1)) + 1;
+                i0 = __ldg(A.deg + 2 * p) * ncell1 + t * (N1 * N2) + b;
+                i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * (N1 * N2) + b;
+                sp = A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+            }
+            const SourceRow src(A, AX, pencil0 + t, p);
 #pragma unroll
             for (int a = 0; a < N1; ++a) {
                 float2 u = make_float2(0.f, 0.f);
@@ -265,6 +287,12 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
                     if (e >= NPURE || !PURE_DIAG) u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
                 }
                 v[a] = u;
+                if (EARLY) {
+                    const float2 own = col[(a * N2) * SI];
+                    float2 ev = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], own, make_float2(0.f, 0.f));
+                    src.add(a * N2 + b, ev);
+                    stg64(sp, stepB * a, ev);
+                }
             }
             if (QC && 32 % (QC ? QC : 1) == 0) __syncwarp();
             else __syncthreads();
@@ -390,7 +418,7 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // ---- tail, specialised kernels: inverse first factor in registers, then one store / vector reduction per element ---------
 // (the coupling was applied in phase 1; every thread owns its column, so there is no barrier and no neighbour data)
 // FIRST: r holds the column's own psi (loaded by tail_load, the first task's before the phase-2 barrier).
-template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG>
+template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG, int AX>
 __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile, const float* sig, long long base, int task,
                                           long long pencil0, float2 (&r)[N1]) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
@@ -409,7 +437,7 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     if (MODE == MODE_FIRST) {
         constexpr int ncell1 = n * (QC / PC) + 1;
         const int i0 = __ldg(A.deg + 2 * p) * ncell1 + t * n + b, i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
-        const SourceRow src(A, pencil0 + t, p);
+        const SourceRow src(A, AX, pencil0 + t, p);
         if (UG) {
             const float2* ab = reinterpret_cast<const float2*>(sig) + t * n + b;
             float g0 = 1.f, g1 = 1.f;
@@ -485,7 +513,7 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
         s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
         s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
     }
-    const SourceRow src(A, pencil0 + t, p);
+    const SourceRow src(A, A.first_axis, pencil0 + t, p);
 #pragma unroll
     for (int a = 0; a < N1; ++a) {
         float2 T = make_float2(0.f, 0.f);
@@ -517,13 +545,16 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
     for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
 }
 
-// UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false>
+// UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance.
+// AX (specialised kernels): the axis of the pass — x tiles of several pencils use the stacked layout, x / y have pure
+// coupling slots, the FIRST pass maps the source box onto its pencils by AX.
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, int VAR = 0>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
+    constexpr bool EARLY = VAR == 1 && MODE == MODE_FIRST && QC != 0;
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
     constexpr bool TMA = QC != 0;                                             // specialised kernels: tile by TMA bulk copies
-    constexpr bool STACKED = TMA && MODE == MODE_FIRST && (QC / (PC ? PC : 1)) > 1;   // x pass (FIRST) with several pencils
+    constexpr bool STACKED = TMA && AX == 0 && (QC / (PC ? PC : 1)) > 1;   // x pass with several pencils per tile
     using G = Geo<N1, N2, QC, PC, STACKED>;
     // couple first needs the rows of one residue owned by a warp (32 % Q == 0) or by one full round of the CTA's task
     // loop (nt % Q == 0, whole rounds); all specialised configurations qualify (checked here at compile time)
@@ -556,21 +587,23 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
     if (first || (!TMA && A.expo)) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
-    phase_fwd1<N1, N2, MODE, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
+    if (EARLY) __syncthreads();                                                          // ... or in phase 1
+    phase_fwd1<N1, N2, AX, E, QC, PC, STACKED, TMA, CF, EARLY>(A, tile, sig, base, valid, tid, nt, bar, pencil0);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
     if constexpr (CF) {
         float2 r[N1];
         // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
         // phase 2 (the loads depend on nothing in shared memory)
-        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
+        constexpr int TMODE = EARLY ? MODE_ACC : MODE;       // EARLY: the tail only adds the streaming term
+        if (TMODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
         __syncthreads();
-        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG>(A, tile, sig, base, tid, pencil0, r);
+        tail_spec<N1, N2, TMODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
-            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG>(A, tile, sig, base, task, pencil0, r2);
+            if (TMODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
+            tail_spec<N1, N2, TMODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();

@@ -4,8 +4,9 @@
 // traffic of a CPU-side Krylov solver).  SURVEY 8(f1).
 //
 // Everything lives on the device: the Krylov basis, the Hessenberg matrix, the Givens rotations, the least-squares
-// right-hand side and the convergence flag.  The host only enqueues kernels and reads ONE double per restart cycle
-// (the true relative residual).  No library: dot products, updates and the small dense algebra are the kernels below.
+// right-hand side and the convergence flag.  The host only enqueues kernels and reads a few scalars per restart cycle
+// (the true relative residual, the Arnoldi step count).  Optionally the system is preconditioned by time stepping:
+// A = I - Phi^s with Phi one SSP-RK3 step of the same transport operator (rte_lib.cu rte_solve_steady).  No library: dot products, updates and the small dense algebra are the kernels below.
 //
 // Arnoldi step k (classical Gram-Schmidt, one fused pass each):
 //   w = L v_k                               three pass kernels (rte_pass.cuh) with the operator tables
@@ -33,13 +34,11 @@ struct Scalars {
     double y[kMaxRestart];                       // least-squares solution of the cycle
     double h[kMaxRestart + 2];                   // folded dot products of the current step (+ norm slot)
     double bnorm, beta, relres, inv;             // ||b||, ||r_0|| of the cycle, residual estimate / ||b||, 1/h_{k+1,k}
-    double tol;
+    double tol;                                  // in-cycle stopping level of the residual estimate / ||b|| (set by the host per cycle)
     int halt, kdone;                             // halt: stop issuing work; kdone: Arnoldi steps completed in this cycle
     int ktotal, pad_;                            // Arnoldi steps completed in all finished cycles
 };
 
-// the tail of Scalars the host reads once per cycle (same member order)
-struct HostView { double bnorm, beta, relres, inv, tol; int halt, kdone, ktotal, pad_; };
 
 __device__ __forceinline__ double block_sum(double v, double* sh) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -169,7 +168,7 @@ __global__ void k_cycle_begin(Scalars* sc, int slot, int first_cycle_sets_bnorm)
     for (int i = 0; i <= kMaxRestart; ++i) sc->g[i] = 0.0;
     sc->g[0] = nrm;
     sc->kdone = 0;
-    sc->halt = (sc->relres <= sc->tol || nrm == 0.0) ? 1 : 0;
+    sc->halt = nrm == 0.0 ? 1 : 0;      // the host decides on convergence between cycles and sets the in-cycle level
     sc->inv = nrm > 0 ? 1.0 / nrm : 0.0;
 }
 
@@ -197,7 +196,7 @@ __global__ void k_givens(Scalars* sc, int k, int norm_slot) {
     // happy breakdown (the Krylov space is exhausted) or converged: stop issuing work
     const bool breakdown = !(hn > 1e-7 * fabs(d));
     sc->inv = breakdown ? 0.0 : 1.0 / hn;
-    if (breakdown || sc->relres <= 0.5 * sc->tol) sc->halt = 1;
+    if (breakdown || sc->relres <= sc->tol) sc->halt = 1;
 }
 
 // end of a cycle: back substitution  R y = g  over the kdone completed steps
