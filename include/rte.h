@@ -174,8 +174,9 @@ int rte_apply_operator(rte_ctx* ctx, const float* x_dev, float* y_dev);
 /* Steady state L psi = q (q = the source of rte_set_source with temporal factor 1) by restarted GMRES(restart),
  * entirely on the device (the paper's Krylov solver was bound by host<->device
  * transfers).  The current state is the initial guess and becomes the solution.  Stops when the TRUE relative
- * residual ||q - L psi|| / ||q||, recomputed at every restart, is <= tol, or after max_restarts cycles (not an
- * error: check *relres_out).  The Krylov basis, the Hessenberg matrix and the rotations live in device memory;
+ * residual ||q - L psi|| / ||q||, recomputed at every restart, is <= tol, after max_restarts cycles, or when that
+ * residual has improved by less than 10 % over three cycles (the fp32 floor, typically 1e-6 .. 1e-5) — neither is an
+ * error: check *relres_out.  The Krylov basis, the Hessenberg matrix and the rotations live in device memory;
  * dot products / updates are this library's kernels; the host reads a few scalars once per restart cycle.
  *   precond_steps = 0: GMRES on L itself.
  *   precond_steps = s > 0: GMRES on the time-stepping fixed-point equation  (I - Phi^s) psi = Phi^s(0; q),  Phi = one

@@ -454,9 +454,9 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     return L;
 }
 
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, int VAR = 0>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0>
 cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
-    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG, AX, VAR>;
+    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG, AX>;
     // the dynamic shared-memory limit is a per-device function attribute: set it once per (kernel instance, device)
     static std::mutex mu;
     static bool configured[64] = {};
@@ -504,16 +504,6 @@ cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaSt
 template <int MODE, int E, int AX>
 cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     constexpr bool F = MODE == rtepass::MODE_FIRST;
-    if constexpr (F && AX == 0) {       // experiment switch: early-store variant of the x pass
-        static const bool early = getenv("RTE_EARLY") && getenv("RTE_EARLY")[0] == '1';
-        if (early && (spec == 0 || spec == 1 || spec == 2)) {
-            PassArgs B = A;
-            B.g_uniform = 0.f;
-            if (spec == 0) return launch_one_impl<24, 16, MODE, E, 32, 32, 256, 2, false, AX, 1>(B, L, s);
-            if (spec == 1) return launch_one_impl<16, 16, MODE, E, 36, 18, 288, 2, false, AX, 1>(B, L, s);
-            return launch_one_impl<16, 8, MODE, E, 32, 8, 256, 3, false, AX, 1>(B, L, s);
-        }
-    }
     switch (spec) {
         case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2, AX>(A, L, s);
         case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3, AX>(A, L, s);
@@ -1309,7 +1299,7 @@ int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, in
     CUDA_TRY(ctx, cudaMemcpyAsync(&hv, (char*)sc + offsetof(Scalars, h) + NT * sizeof(double), sizeof(Host), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     const double qnorm = std::sqrt(hv.h64);
-    double relres = 0.0;
+    double relres = 0.0, history[3] = {0, 0, 0}, past3 = 1e300;
     int cycles = 0;
     if (!(qnorm > 0.0)) {                                      // q = 0: the steady state is psi = 0
         CUDA_TRY(ctx, cudaMemsetAsync(ctx->psi, 0, fb, st));
@@ -1334,6 +1324,11 @@ int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, in
             CUDA_TRY(ctx, cudaStreamSynchronize(st));
             relres = s > 0 ? std::sqrt(hv.h64) / qnorm : hv.relres;
             if (!(relres > tol) || cycle == max_restarts || !(hv.relres > 0.0)) break;
+            // stagnation (the fp32 floor of the true residual, or a diverging preconditioner step): less than 1 % gained
+            // over the last three cycles
+            history[cycle % 3] = relres;
+            if (cycle >= 3 && relres > 0.99 * past3) break;
+            past3 = history[(cycle + 1) % 3];                  // the value from two cycles ago becomes "three ago" next time
             // in-cycle stopping level for the device (relative to ||b||): the residual of the solved system has to fall by
             // tol / relres; with a preconditioner its norm is not the true one, so aim a little lower
             const double level = (s > 0 ? 0.3 : 1.0) * tol / relres * hv.relres;

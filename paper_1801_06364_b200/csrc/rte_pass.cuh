@@ -233,12 +233,9 @@ struct SourceRow {
 // one shared-memory store and E loads per element become E loads, and the tail runs without any barrier.  The
 // gather reads rows that other columns of the same rows overwrite, hence the fence between gather and store: the rows
 // of one residue b are owned by one warp (32 % Q == 0) or by one round of the whole CTA (nt % Q == 0).
-// EARLY (FIRST pass, experiment): the column's own psi is still in the tile during the gather, so the Euler diagonal
-// and the source are applied HERE and stored to the new buffer at once; the tail then adds -c dt T_x by a vector
-// reduction like the accumulating passes (same thread, same address: program order) instead of re-reading psi.
-template <int N1, int N2, int AX, int E, int QC, int PC, bool STACKED, bool TMA, bool CF, bool EARLY = false>
+template <int N1, int N2, int AX, int E, int QC, int PC, bool STACKED, bool TMA, bool CF>
 __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, const float* sig, long long base, int valid,
-                                           int tid, int nt, unsigned long long* bar, long long pencil0 = 0) {
+                                           int tid, int nt, unsigned long long* bar) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     const int P = PC ? PC : A.P;
     const int Q = QC ? QC : A.TP * P;
@@ -267,15 +264,6 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
                 ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
             }
             mbar_wait(bar + (STACKED ? 0 : b), 0);
-            int i0 = 0, i1 = 0;
-            float2* sp = nullptr;
-            if (EARLY) {
-                constexpr int ncell1 = (N1 * N2) * (QC / (PC ? PC : 1)) + 1;
-                i0 = __ldg(A.deg + 2 * p) * ncell1 + t * (N1 * N2) + b;
-                i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * (N1 * N2) + b;
-                sp = A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
-            }
-            const SourceRow src(A, AX, pencil0 + t, p);
 #pragma unroll
             for (int a = 0; a < N1; ++a) {
                 float2 u = make_float2(0.f, 0.f);
@@ -287,12 +275,6 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
                     if (e >= NPURE || !PURE_DIAG) u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
                 }
                 v[a] = u;
-                if (EARLY) {
-                    const float2 own = col[(a * N2) * SI];
-                    float2 ev = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], own, make_float2(0.f, 0.f));
-                    src.add(a * N2 + b, ev);
-                    stg64(sp, stepB * a, ev);
-                }
             }
             if (QC && 32 % (QC ? QC : 1) == 0) __syncwarp();
             else __syncthreads();
@@ -548,9 +530,8 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
 // UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance.
 // AX (specialised kernels): the axis of the pass — x tiles of several pencils use the stacked layout, x / y have pure
 // coupling slots, the FIRST pass maps the source box onto its pencils by AX.
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, int VAR = 0>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0>
 __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
-    constexpr bool EARLY = VAR == 1 && MODE == MODE_FIRST && QC != 0;
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
     constexpr bool TMA = QC != 0;                                             // specialised kernels: tile by TMA bulk copies
@@ -587,23 +568,21 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
     }
     if (first || (!TMA && A.expo)) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
-    if (EARLY) __syncthreads();                                                          // ... or in phase 1
-    phase_fwd1<N1, N2, AX, E, QC, PC, STACKED, TMA, CF, EARLY>(A, tile, sig, base, valid, tid, nt, bar, pencil0);
+    phase_fwd1<N1, N2, AX, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
     if constexpr (CF) {
         float2 r[N1];
         // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
         // phase 2 (the loads depend on nothing in shared memory)
-        constexpr int TMODE = EARLY ? MODE_ACC : MODE;       // EARLY: the tail only adds the streaming term
-        if (TMODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
+        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
         __syncthreads();
-        tail_spec<N1, N2, TMODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, tid, pencil0, r);
+        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            if (TMODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
-            tail_spec<N1, N2, TMODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, task, pencil0, r2);
+            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
+            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();
