@@ -389,19 +389,19 @@ int check_grid(const rte_grid* g) {
 // configurations — or the generic kernel (run-time P, TP, block size, FIRST/ACC) for every other supported extent / order.
 struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; };
 
-struct SpecRow { int n, P, TP, nt; };
+struct SpecRow { int n, P, TP, nt, TPx; };   // TP: pencils per y / z tile, TPx: per x tile
 constexpr SpecRow kSpec[] = {
-    {384, 32, 1, 256},   // cfg4: 384^3 P_7   (98 KB tile, 2 CTAs / SM)
-    {256, 18, 2, 288},   // cfg3: 256^3 P_5   (288 B chunks = 9 whole sectors)
-    {128, 8, 4, 256},    // cfg2: 128^3 P_3
-    {512, 8, 2, 256},    // cfg1: 512^2 P_7 (2-D)
-    {64, 4, 8, 256},     // cfg0: 64^2 P_3 (2-D)
-    {64, 32, 1, 256},    // the paper's second run: 64^3 P_7
+    {384, 32, 1, 256, 1},   // cfg4: 384^3 P_7   (98 KB tile, 2 CTAs / SM)
+    {256, 18, 2, 288, 2},   // cfg3: 256^3 P_5   (288 B chunks = 9 whole sectors)
+    {128, 8, 4, 256, 4},    // cfg2: 128^3 P_3
+    {512, 8, 2, 256, 2},    // cfg1: 512^2 P_7 (2-D)
+    {64, 4, 8, 256, 8},     // cfg0: 64^2 P_3 (2-D)
+    {64, 32, 1, 256, 1},    // the paper's second run: 64^3 P_7
 };
 
 size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
     size_t b = (size_t)n * Q * sizeof(float2);
-    if (diag) b += (size_t)nsig * ((size_t)n * TP + 1) * sizeof(float);   // per-tile table of the Euler diagonal
+    if (diag) b += (size_t)nsig * (size_t)rtepass::sig_pitch_l(n, TP) * sizeof(float);   // per-tile table of the Euler diagonal
     return b;
 }
 
@@ -423,12 +423,14 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     L.spec = -1;
     A.P = P;
     if (kind != KIND_EXP)                          // the exponential step runs on the generic kernels
-        for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s)
-            if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % kSpec[s].TP == 0 &&
+        for (int s = 0; s < (int)(sizeof(kSpec) / sizeof(kSpec[0])); ++s) {
+            const int tp = axis == 0 ? kSpec[s].TPx : kSpec[s].TP;
+            if (kSpec[s].n == n && kSpec[s].P == P && A.pencils_per_group % tp == 0 &&
                 !(axis == 2 && T.maxcnt > 2) && !(axis < 2 && T.npure < 2)) {
-                L.spec = s; L.TP = kSpec[s].TP; L.nt = kSpec[s].nt;
+                L.spec = s; L.TP = tp; L.nt = kSpec[s].nt;
                 break;
             }
+        }
     if (L.spec < 0) {
         int tp = 1;
         while (tp * P < 32 && tp < 8) tp *= 2;

@@ -295,7 +295,9 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
 }
 
 // ---- phase 2: twiddle, second factor forward, i k / n, second factor inverse, conjugate twiddle -----------------------
-template <int N1, int N2, int QC, int PC, bool STACKED>
+// LOWREG (instances that run 3+ CTAs per SM): the twiddles are fetched again for the conjugate multiply instead of
+// being kept in N2 register pairs across the two transforms (constant-cache reads, off the load/store data path).
+template <int N1, int N2, int QC, int PC, bool STACKED, bool LOWREG = false>
 __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int tid, int nt) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
     constexpr int n = N1 * N2;
@@ -311,9 +313,12 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
         float2 v[N2], w[N2];
 #pragma unroll
         for (int b = 0; b < N2; ++b) v[b] = row[b * SI];
+        int ti = 0;     // running twiddle index k1*b; LOWREG pins it so that the N2 indices are not precomputed and spilled
 #pragma unroll
         for (int b = 1; b < N2; ++b) {
-            w[b] = CT ? c_tw[off + k1 * b] : __ldg(A.tw + k1 * b);
+            ti += k1;
+            if (LOWREG) asm volatile("" : "+r"(ti));
+            w[b] = CT ? c_tw[off + ti] : __ldg(A.tw + ti);
             v[b] = rtefft::cmul(v[b], w[b]);
         }
         rtefft::dft_fwd<N2>(v);
@@ -326,8 +331,14 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
             v[k2] = rtefft::cscale(make_float2(-v[k2].y, v[k2].x), kw);
         }
         rtefft::dft_inv<N2>(v);
+        ti = 0;
 #pragma unroll
-        for (int b = 1; b < N2; ++b) v[b] = rtefft::cmulc(v[b], w[b]);
+        for (int b = 1; b < N2; ++b) {
+            ti += k1;
+            if (LOWREG) asm volatile("" : "+r"(ti));
+            const float2 wc = LOWREG ? (CT ? c_tw[off + ti] : __ldg(A.tw + ti)) : w[b];
+            v[b] = rtefft::cmulc(v[b], wc);
+        }
 #pragma unroll
         for (int b = 0; b < N2; ++b) row[b * SI] = v[b];
     }
@@ -353,10 +364,23 @@ __device__ __forceinline__ void phase_inv1(const PassArgs& A, float2* tile, int 
     }
 }
 
+// Pitches of the per-tile diagonal table sig[l*sig_pitch_l + t*sig_pitch_t + i] (floats).  A reading warp spans degrees l,
+// (with several pencils per tile) pencils t and, when a tile row is not a multiple of 32 columns, two neighbouring cells
+// i: with the pencil pitch = 2 and the degree pitch = 4 (mod 32 banks) the lanes' banks 4 l + 2 t + {0, 1} are distinct for up
+// to 8 degrees and 2 pencils (every BASELINE configuration); other shapes stay correct and may conflict.
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int sig_pitch_t(int n) { return n + 2; }
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int sig_pitch_l(int n, int TP) { return TP * (n + 2) + (36 - (TP * (n + 2)) % 32) % 32; }
+
 // ---- FIRST only: per-tile table of the Euler diagonal  s_l(r) = 1 - c dt sigma_l(r) -----------------------------------
 // sigma_l = mu_a + mu_s (1 - g^l) in Omega (eq.(9); g^l by repeated multiplication, R16),
 //         = mu_b for every l in the PML, where the maps hold (mu_b, 0, g) (eq.(12)).
-// Layout sig[l*(ncell+1) + j], j = t*n + i: conflict-free to build (lanes = cells) and to read (lanes = degrees).
+// Layout sig[l*sig_pitch_l + t*sig_pitch_t + i]: conflict-free to build (lanes = cells) and to read (lanes = degrees, pencils).
 // (General form s_l = ident - c dt sigma_l: ident = 1 for a time step; ident = 0, c dt = -1 gives s_l = sigma_l, the
 // diagonal of the steady-state operator L = T + sigma_l; expo: s_l = exp(-c dt sigma_l), generic kernels only.)
 // Uniform g (A.g_uniform > 0): s_l = 1 - c dt (sa + ss (1 - g^l)) = A + B g^l with A = 1 - c dt (sa + ss), B = c dt ss,
@@ -379,6 +403,7 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
         }
         return;
     }
+    const int pl = sig_pitch_l(n, A.TP);
     for (int j = tid; j < ncell; j += nt) {
         const int t = j / n, i = j - t * n;
         float sa = 0.f, ss = 0.f, g = 0.f;
@@ -387,12 +412,12 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
             sa = __ldg(A.sa + cell); ss = __ldg(A.ss + cell); g = __ldg(A.gm + cell);
         }
         float pw = 1.f;
-        float* dst = sig + j;
+        float* dst = sig + t * sig_pitch_t(n) + i;
         for (int l = 0; l < A.nsig; ++l) {
             const float a = A.cdt * fmaf(ss, 1.f - pw, sa);          // c dt sigma_l
             *dst = A.expo ? expf(-a) : A.ident - a;                  // exponential step: exact decay over the step
             pw *= g;
-            dst += ncell + 1;
+            dst += pl;
         }
     }
 }
@@ -415,47 +440,77 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
     if (MODE == MODE_FIRST) rtefft::dft_inv_swap<N1>(v);      // register pressure: see rte_fft.cuh
     else rtefft::dft_inv<N1>(v);
-    float2* sp = A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    // x pass (AX == 0): the pencil is contiguous (cell stride 1, pencil stride n), so every address of the column is the
+    // base plus a compile-time offset and folds into the instruction's immediate field
+    float2* sp = AX == 0 ? A.acc + (base + (long long)t * n + b) * P + p
+                         : A.acc + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    auto store = [&](int a, float2 e) {
+        if (AX == 0) sp[a * (N2 * P)] = e;
+        else stg64(sp, stepB * a, e);
+    };
     if (MODE == MODE_FIRST) {
-        constexpr int ncell1 = n * (QC / PC) + 1;
-        const int i0 = __ldg(A.deg + 2 * p) * ncell1 + t * n + b, i1 = __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
+        constexpr int pl = sig_pitch_l(n, QC / PC), pt = sig_pitch_t(n);
+        const int i0 = __ldg(A.deg + 2 * p) * pl + t * pt + b, i1 = __ldg(A.deg + 2 * p + 1) * pl + t * pt + b;
         const SourceRow src(A, AX, pencil0 + t, p);
+        // (the source test is hoisted out of the element loops: almost every pencil lies outside the source box)
         if (UG) {
             const float2* ab = reinterpret_cast<const float2*>(sig) + t * n + b;
             float g0 = 1.f, g1 = 1.f;
             for (int l = __ldg(A.deg + 2 * p); l > 0; --l) g0 *= A.g_uniform;          // g^l by repeated multiplication (R16)
             for (int l = __ldg(A.deg + 2 * p + 1); l > 0; --l) g1 *= A.g_uniform;
+            if (src.on) {
 #pragma unroll
-            for (int a = 0; a < N1; ++a) {
-                const float2 c = ab[a * N2];
-                float2 e = rtefft::cfma_diag(fmaf(c.y, g0, c.x), fmaf(c.y, g1, c.x), r[a], v[a]);
-                src.add(a * N2 + b, e);
-                stg64(sp, stepB * a, e);
+                for (int a = 0; a < N1; ++a) {
+                    const float2 c = ab[a * N2];
+                    float2 e = rtefft::cfma_diag(fmaf(c.y, g0, c.x), fmaf(c.y, g1, c.x), r[a], v[a]);
+                    src.add(a * N2 + b, e);
+                    store(a, e);
+                }
+            } else {
+#pragma unroll
+                for (int a = 0; a < N1; ++a) {
+                    const float2 c = ab[a * N2];
+                    store(a, rtefft::cfma_diag(fmaf(c.y, g0, c.x), fmaf(c.y, g1, c.x), r[a], v[a]));
+                }
             }
-        } else {
+        } else if (src.on) {
 #pragma unroll
             for (int a = 0; a < N1; ++a) {
                 float2 e = rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], r[a], v[a]);
                 src.add(a * N2 + b, e);
-                stg64(sp, stepB * a, e);
+                store(a, e);
             }
+        } else {
+#pragma unroll
+            for (int a = 0; a < N1; ++a) store(a, rtefft::cfma_diag(sig[i0 + a * N2], sig[i1 + a * N2], r[a], v[a]));
         }
     } else {
+        // one running pointer instead of N1 precomputed 64-bit addresses (they would not fit the 3-CTA register budget)
+        unsigned long long off = 0;
 #pragma unroll
-        for (int a = 0; a < N1; ++a) red_add64(sp, stepB * a, v[a]);
+        for (int a = 0; a < N1; ++a) {
+            red_add64(sp, off, v[a]);
+            asm volatile("add.u64 %0, %0, %1;" : "+l"(off) : "l"(stepB));
+        }
     }
 }
 
 // the psi re-read of one FIRST tail task, issued as early as possible
-template <int N1, int N2, int QC, int PC>
+template <int N1, int N2, int QC, int PC, int AX>
 __device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]) {
     constexpr int P = PC, Q = QC;
-    const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
     const int b = task / Q, q = task - b * Q;
     const int t = q / P, p = q - t * P;
-    const float2* lp = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+    if (AX == 0) {          // x pass: compile-time offsets (see tail_spec)
+        const float2* lp = A.psi + (base + (long long)t * (N1 * N2) + b) * P + p;
 #pragma unroll
-    for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+        for (int a = 0; a < N1; ++a) r[a] = lp[a * (N2 * P)];
+    } else {
+        const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
+        const float2* lp = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
+#pragma unroll
+        for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+    }
 }
 
 // ---- tail, generic kernels: coupling from the differentiated pencil + accumulate / integrate -----------------------------
@@ -491,9 +546,9 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
     const float* s1 = sig;
     const bool table = first || A.expo;
     if (table) {
-        const int ncell1 = n * A.TP + 1;
-        s0 = sig + __ldg(A.deg + 2 * p) * ncell1 + t * n + b;
-        s1 = sig + __ldg(A.deg + 2 * p + 1) * ncell1 + t * n + b;
+        const int pl = sig_pitch_l(n, A.TP), pt = sig_pitch_t(n);
+        s0 = sig + __ldg(A.deg + 2 * p) * pl + t * pt + b;
+        s1 = sig + __ldg(A.deg + 2 * p + 1) * pl + t * pt + b;
     }
     const SourceRow src(A, A.first_axis, pencil0 + t, p);
 #pragma unroll
@@ -570,18 +625,18 @@ __global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __gri
     if (first || (!TMA && A.expo)) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
     phase_fwd1<N1, N2, AX, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
     __syncthreads();
-    phase_mid<N1, N2, QC, PC, STACKED>(A, tile, tid, nt);
+    phase_mid<N1, N2, QC, PC, STACKED, (MINB >= 3 && N2 >= 16)>(A, tile, tid, nt);
     if constexpr (CF) {
         float2 r[N1];
         // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
         // phase 2 (the loads depend on nothing in shared memory)
-        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, tid, r);
+        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC, AX>(A, base, tid, r);
         __syncthreads();
         tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC>(A, base, task, r2);
+            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC, AX>(A, base, task, r2);
             tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
