@@ -439,7 +439,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
         const int Q = tp * P;
         const int T1 = Q * T.N2, T2 = Q * T.N1;
         int best = 128; double best_cost = 1e30;
-        const int ntmax = T.N1 > 32 ? 224 : 320;   // 36-point register transforms: 255 registers x 224 threads fit one SM
+        const int ntmax = rtepass::generic_max_threads(T.N1, T.N2);   // by register need of the transforms (rte_pass.cuh)
         for (int nt = 64; nt <= ntmax; nt += 32) {
             if (nt > T1 && nt > T2 && nt > 64) break;
             const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;

@@ -537,11 +537,14 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
         ws[e] = __ldg(reinterpret_cast<const float2*>(&ce->ws0));
     }
     const long long gi = (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
-    const float2* lp = (first ? A.psi : A.acc) + gi;
     float2* sp = A.acc + gi;
     float2 r[N1];
+    // FIRST re-reads psi; the accumulating passes add their term by a fire-and-forget vector reduction like the
+    // specialised kernels (one reduction per address per pass: deterministic), so they load nothing here
+    if (first) {
 #pragma unroll
-    for (int a = 0; a < N1; ++a) r[a] = ldg64(lp, stepB * a);
+        for (int a = 0; a < N1; ++a) r[a] = ldg64(A.psi + gi, stepB * a);
+    }
     const float* s0 = sig;
     const float* s1 = sig;
     const bool table = first || A.expo;
@@ -569,24 +572,38 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
                 if (qv.x != 0.f) r[a].x = fmaf(e0 < 1.f ? (1.f - e0) / -logf(e0) : 1.f, qv.x, r[a].x);
                 if (qv.y != 0.f) r[a].y = fmaf(e1 < 1.f ? (1.f - e1) / -logf(e1) : 1.f, qv.y, r[a].y);
             } else {
-                r[a] = rtefft::cfma_diag(e0, e1, T, r[a]);
+                r[a] = make_float2(e0 * T.x, e1 * T.y);
             }
         } else if (first) {
             r[a] = rtefft::cfma_diag(s0[a * N2], s1[a * N2], r[a], T);
             src.add(a * N2 + b, r[a]);
         } else {
-            r[a] = rtefft::cadd(r[a], T);
+            r[a] = T;
         }
     }
+    if (first) {
 #pragma unroll
-    for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
+        for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
+    } else {
+#pragma unroll
+        for (int a = 0; a < N1; ++a) red_add64(sp, stepB * a, r[a]);
+    }
+}
+
+// Largest block of a generic instance: small register transforms leave room for more threads (a tile of many
+// coefficients allows one CTA per SM only, so the block is the occupancy), 32/36-point ones need their 255 registers.
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int generic_max_threads(int N1, int N2) {
+    return (N1 > 32 || N2 > 32) ? 224 : ((N1 > 24 || N2 > 24) ? 256 : ((N1 > 18 || N2 > 18) ? 320 : ((N1 > 9 || N2 > 12) ? 512 : 640)));
 }
 
 // UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance.
 // AX (specialised kernels): the axis of the pass — x tiles of several pencils use the stacked layout, x / y have pure
 // coupling slots, the FIRST pass maps the source box onto its pencils by AX.
 template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0>
-__global__ void __launch_bounds__(NTC ? NTC : 320, MINB) pass_kernel(const __grid_constant__ PassArgs A) {
+__global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB) pass_kernel(const __grid_constant__ PassArgs A) {
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
     constexpr bool TMA = QC != 0;                                             // specialised kernels: tile by TMA bulk copies
