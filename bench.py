@@ -358,7 +358,9 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {"cfg4": {0: 29695333000, 1: 43428661000, 2: 43432189000}}   # profiles/r1f_pass_kernels.md
+TRAFFIC_NCU = {"cfg4": {0: 29696323999, 1: 43428465000, 2: 43432492000},       # profiles/r2j_summary.md §3 (ncu --set full,
+               "cfg3": {0: 4991200000, 1: 7194781000, 2: 7201715000},          # one launch per axis kernel)
+               "cfg2": {0: 246044416, 1: 344825344, 2: 345956864}}
 
 
 def max_over_ranks(ms, dist, device):
@@ -624,8 +626,9 @@ def run_ours(args, wl, cfg):
             rf = roofline_of(c2, r2, peak, peak_kind)
             others[name] = {"ms_per_step": r2["ms"] / DEFAULT_STEPS[name],
                             "value": c2.C * c2.G * DEFAULT_STEPS[name] / (r2["ms"] * 1e-3),
-                            "whole_step_frac": rf["whole_step"]["frac"], "dominant_kernel_frac": rf["frac"],
-                            "finite": r2["finite"]}
+                            "whole_step_frac": rf["whole_step"]["frac"],
+                            "whole_step_frac_of_nominal_8000": rf["whole_step"]["frac_of_nominal_8000"],
+                            "dominant_kernel_frac": rf["frac"], "finite": r2["finite"]}
             del r2
             torch.cuda.empty_cache()
         line["other_3d_workloads"] = others

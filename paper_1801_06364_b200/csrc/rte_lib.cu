@@ -1364,7 +1364,7 @@ int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, in
     return RTE_OK;
 }
 
-int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host) {
+static int step_profile_impl(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host) {
     if (!ctx) return RTE_ESTATE;
     if (nsteps < 0 || !ms_axis_host) return fail(ctx, RTE_EINVAL, "bad rte_step_profile argument");
     const int naxes = ctx->grid.dim;
@@ -1391,6 +1391,10 @@ int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* 
             }
     for (auto& e : ev) cudaEventDestroy(e);
     return rc;
+}
+
+int rte_step_profile(rte_ctx* ctx, int nsteps, double* ms_axis_host, long long* launches_axis_host) {
+    return guarded([&]() -> int { return step_profile_impl(ctx, nsteps, ms_axis_host, launches_axis_host); });
 }
 
 int rte_fluence(rte_ctx* ctx, float* phi_dev) {

@@ -227,3 +227,46 @@ def test_cufft_literal_reference_point_vs_oracle_literal(shape, N):
     o.set_state(psi0)
     o.step(5, orc.LITERAL)
     assert_parity(got, o.get_state(), f"cufft literal {shape} P{N}")
+
+
+def test_graph_survives_source_changes_and_other_integrators():
+    """The captured launches hold the source box by value and the state buffers by address: rte_set_source drops the graph,
+    and a step of another integrator (which leaves the state in a different buffer) must not let a replay read stale data."""
+    cfg, mu_a, mu_s, g, src = random_case(2, 64, 48, 1, 3, dx=0.1, dt=0.001, W=4)
+    rng = np.random.default_rng(77)
+    src2 = dict(w=rng.standard_normal(cfg.C).astype(np.float32), S=rng.standard_normal((1, 9, 11)).astype(np.float32),
+                origin=(20, 10, 0), extent=(11, 9, 1), kind=1, t0=0.0, sigma_t=1.0)
+    psi0 = wl.random_state(cfg, seed=6)
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    rte.rte_set_state(ctx, dev(psi0))
+    o.set_state(psi0)
+    for s_ in (src, src2):
+        rte.rte_set_source(ctx, s_["w"], dev(s_["S"]), s_["origin"], s_["extent"], s_["kind"], s_["t0"], s_["sigma_t"])
+        o.set_source(s_["w"], s_["S"], s_["origin"], s_["extent"], s_["kind"], s_["t0"], s_["sigma_t"])
+        rte.rte_step(ctx, 70)                 # graph replays
+        o.step(70)
+        rte.rte_step_ssprk3(ctx, 1)           # leaves the state in the other buffer
+        o.step_ssprk3(1)
+        rte.rte_step(ctx, 41)                 # replays again: must pick up the right buffer
+        o.step(41)
+    assert_parity(gpu_state(ctx, cfg), o.get_state(), "graph + source change + ssprk3")
+    assert abs(rte.rte_time_ps(ctx) - o.time_ps()) < 1e-6
+
+
+def test_solve_steady_2d_vs_oracle():
+    """2-D steady state (circular harmonics P_4, disks, PML, constant source), preconditioned GMRES vs the oracle's GMRES."""
+    cfg = wl.reduced(wl.CONFIGS["cfg1"], 64, pml_width=6, dx=0.25)
+    cfg = wl.replace(cfg, N=4, n_inclusions=5)
+    mu_a, mu_s, g = wl.media_maps(cfg)
+    w = np.zeros(cfg.C, np.float32); w[0] = 1.0; w[1] = 0.5
+    S = np.ones((1, 3, 3), np.float32)
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    rte.rte_set_source(ctx, w, dev(S), (30, 31, 0), (3, 3, 1), 1)
+    napp, rr = rte.rte_solve_steady(ctx, restart=20, tol=2e-6, max_restarts=60, precond_steps=6,
+                                    precond_dt_ps=0.3 * cfg.dx / cfg.c)
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_source(w, S, (30, 31, 0), (3, 3, 1), 1)
+    _, orr = o.solve_steady(restart=40, tol=1e-10, max_restarts=200)
+    assert orr <= 1e-10 and rr <= 2e-6, (rr, orr)
+    assert_parity(gpu_state(ctx, cfg), o.get_state(), f"2-D steady ({napp} sweeps)")
