@@ -386,30 +386,46 @@ constexpr int sig_pitch_l(int n, int TP) { return TP * (n + 2) + (36 - (TP * (n 
 // Uniform g (A.g_uniform > 0): s_l = 1 - c dt (sa + ss (1 - g^l)) = A + B g^l with A = 1 - c dt (sa + ss), B = c dt ss,
 // so the table holds the float2 (A, B) per cell and every thread keeps g^l of its two slots in registers: one
 // broadcast 8-byte read per element instead of two 4-byte reads, and a quarter of the table-building work.
-template <int N1, int N2>
-__device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long long base, int valid, int tid, int nt) {
+// The map values of the (at most MAXC) cells a thread is responsible for; loaded BEFORE the TMA issue loop so that their DRAM
+// latency overlaps it (ncu: the first use of these loads was the kernel's hottest stall).
+template <int MAXC>
+struct SigCells { float sa[MAXC], ss[MAXC], g[MAXC]; };
+
+template <int N1, int N2, int MAXC>
+__device__ __forceinline__ void load_sig_cells(const PassArgs& A, SigCells<MAXC>& c, long long base, int valid, int tid, int nt) {
     constexpr int n = N1 * N2;
     const int ncell = n * A.TP;
-    if (A.g_uniform > 0.f) {
-        float2* ab = reinterpret_cast<float2*>(sig);
-        for (int j = tid; j < ncell; j += nt) {
+#pragma unroll
+    for (int k = 0; k < MAXC; ++k) {
+        const int j = tid + k * nt;
+        c.sa[k] = c.ss[k] = c.g[k] = 0.f;
+        if (j < ncell) {
             const int t = j / n, i = j - t * n;
-            float sa = 0.f, ss = 0.f;
             if (t < valid) {
                 const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
-                sa = __ldg(A.sa + cell); ss = __ldg(A.ss + cell);
+                c.sa[k] = __ldg(A.sa + cell); c.ss[k] = __ldg(A.ss + cell);
+                if (!(A.g_uniform > 0.f)) c.g[k] = __ldg(A.gm + cell);
             }
-            ab[j] = make_float2(A.ident - A.cdt * (sa + ss), A.cdt * ss);
         }
-        return;
     }
+}
+
+template <int N1, int N2, int MAXC>
+__device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, const SigCells<MAXC>& c, int tid, int nt) {
+    constexpr int n = N1 * N2;
+    const int ncell = n * A.TP;
+    const bool ug = A.g_uniform > 0.f;
+    float2* ab = reinterpret_cast<float2*>(sig);
     const int pl = sig_pitch_l(n, A.TP);
-    for (int j = tid; j < ncell; j += nt) {
+#pragma unroll
+    for (int k = 0; k < MAXC; ++k) {
+        const int j = tid + k * nt;
+        if (j >= ncell) break;
         const int t = j / n, i = j - t * n;
-        float sa = 0.f, ss = 0.f, g = 0.f;
-        if (t < valid) {
-            const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
-            sa = __ldg(A.sa + cell); ss = __ldg(A.ss + cell); g = __ldg(A.gm + cell);
+        const float sa = c.sa[k], ss = c.ss[k], g = c.g[k];
+        if (ug) {
+            ab[j] = make_float2(A.ident - A.cdt * (sa + ss), A.cdt * ss);
+            continue;
         }
         float pw = 1.f;
         float* dst = sig + t * sig_pitch_t(n) + i;
@@ -419,6 +435,26 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
             pw *= g;
             dst += pl;
         }
+    }
+}
+
+// generic kernels (run-time tile size): load and build in one loop
+template <int N1, int N2>
+__device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long long base, int valid, int tid, int nt) {
+    for (int j0 = 0; j0 < N1 * N2 * A.TP; j0 += nt) {
+        SigCells<1> c;
+        // (tid + j0: one cell per thread and round)
+        const int n = N1 * N2, j = tid + j0;
+        c.sa[0] = c.ss[0] = c.g[0] = 0.f;
+        if (j < n * A.TP) {
+            const int t = j / n, i = j - t * n;
+            if (t < valid) {
+                const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
+                c.sa[0] = __ldg(A.sa + cell); c.ss[0] = __ldg(A.ss + cell);
+                if (!(A.g_uniform > 0.f)) c.g[0] = __ldg(A.gm + cell);
+            }
+        }
+        build_sig<N1, N2, 1>(A, sig, c, tid + j0, nt);
     }
 }
 
@@ -607,7 +643,10 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
     constexpr bool TMA = QC != 0;                                             // specialised kernels: tile by TMA bulk copies
-    constexpr bool STACKED = TMA && AX == 0 && (QC / (PC ? PC : 1)) > 1;   // x pass with several pencils per tile
+    // x pass: pencils are contiguous in memory -> the tile is filled by a few large bulk copies ("stacked" layout; with
+    // one pencil per tile it coincides with the interleaved one).  ncu: the 384 per-row copies of the one-pencil x tile
+    // cost 8 % of the kernel's stall samples in their lane-serialised issue loop.
+    constexpr bool STACKED = TMA && AX == 0;
     using G = Geo<N1, N2, QC, PC, STACKED>;
     // couple first needs the rows of one residue owned by a warp (32 % Q == 0) or by one full round of the CTA's task
     // loop (nt % Q == 0, whole rounds); all specialised configurations qualify (checked here at compile time)
@@ -632,14 +671,19 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
     const long long base = group * A.group_stride + (long long)tin * A.TP * A.stride_t;
     const long long pencil0 = (long long)blockIdx.x * A.TP;
     if constexpr (TMA) {
+        constexpr int MAXC = (n * (QC / (PC ? PC : 1)) + (NTC ? NTC : 1) - 1) / (NTC ? NTC : 1);
+        SigCells<MAXC> cells;
+        if (MODE == MODE_FIRST) load_sig_cells<N1, N2, MAXC>(A, cells, base, valid, tid, nt);   // in flight during the TMA issue
         if (tid < NBAR) {
             mbar_init(&bar[tid], 1);
             mbar_arrive_expect_tx(&bar[tid], (unsigned)(n / NBAR) * QC * 8u);
         }
         __syncthreads();
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
+        if (MODE == MODE_FIRST) build_sig<N1, N2, MAXC>(A, sig, cells, tid, nt);                 // read in the tail, two barriers later
+    } else {
+        if (first || A.expo) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
     }
-    if (first || (!TMA && A.expo)) build_sig<N1, N2>(A, sig, base, valid, tid, nt);     // read in the tail, two barriers later
     phase_fwd1<N1, N2, AX, E, QC, PC, STACKED, TMA, CF>(A, tile, sig, base, valid, tid, nt, bar);
     __syncthreads();
     phase_mid<N1, N2, QC, PC, STACKED, (MINB >= 3 && N2 >= 16)>(A, tile, tid, nt);
