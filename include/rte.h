@@ -237,6 +237,17 @@ int rte_media_ellipsoids(const rte_grid* grid, float dx_mm, const float backgrou
 int rte_media_lognormal(const rte_grid* grid, float dx_mm, uint64_t seed, float mean, float sigma_log,
                         float corr_len_mm, float* out_dev, float* scratch_dev, void* cuda_stream);
 
+/* rte_media_lognormal for callers that cannot allocate device memory (CUDA-graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same field, same kernels, but the blur scratch and the reduction scalars live in one static device
+ * array inside the library (8 MiB + 256 B per GPU, held from library load until exit) instead of caller scratch and a
+ * cudaMalloc.  Calls no cudaMalloc / cudaFree / allocating routine and does not synchronise: asynchronous on the stream.
+ * Limit: nx*ny*nz <= 2 097 152 cells (128^3); larger grids return RTE_EUNSUPPORTED (text in rte_last_error(NULL)).
+ * All calls on one GPU share that array: calls that overlap on the GPU (different streams) race — serialise them.  The
+ * array keeps the previous call's contents; the entry point clears what must start at zero itself.  (The first call
+ * on a device resolves the array's address with cudaGetSymbolAddress: make it outside a capture.) */
+int rte_media_lognormal_noalloc(const rte_grid* grid, float dx_mm, uint64_t seed, float mean, float sigma_log,
+                                float corr_len_mm, float* out_dev, void* cuda_stream);
+
 /* The PML profile alone (mu_b per cell, 0 inside Omega) and the Omega mask (1 inside), device outputs. */
 int rte_pml_profile(const rte_grid* grid, const rte_pml* pml, float* mu_b_dev, unsigned char* inside_dev,
                     void* cuda_stream);

@@ -74,6 +74,7 @@ _lib.rte_launch_count.argtypes = [_vp, C.POINTER(C.c_longlong)]
 _lib.rte_media_ellipsoids.argtypes = [C.POINTER(rte_grid), _f, C.POINTER(C.c_float), _i, C.POINTER(C.c_float), _vp,
                                       _vp, _vp, _vp]
 _lib.rte_media_lognormal.argtypes = [C.POINTER(rte_grid), _f, C.c_uint64, _f, _f, _f, _vp, _vp, _vp]
+_lib.rte_media_lognormal_noalloc.argtypes = [C.POINTER(rte_grid), _f, C.c_uint64, _f, _f, _f, _vp, _vp]
 _lib.rte_pml_profile.argtypes = [C.POINTER(rte_grid), C.POINTER(rte_pml), _vp, _vp, _vp]
 
 EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_workspace_bytes", "rte_create", "rte_destroy",
@@ -82,7 +83,7 @@ EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_w
             "rte_extra_workspace_bytes", "rte_set_extra_workspace", "rte_stable_dt", "rte_apply_operator",
             "rte_solve_steady", "rte_fluence", "rte_fluence_host",
             "rte_fluence_change", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
-            "rte_media_ellipsoids", "rte_media_lognormal", "rte_pml_profile"]
+            "rte_media_ellipsoids", "rte_media_lognormal", "rte_media_lognormal_noalloc", "rte_pml_profile"]
 
 
 def _check(rc, ctx=None):
@@ -370,6 +371,13 @@ def rte_media_lognormal(grid, dx_mm, seed, mean, sigma_log, corr_len_mm, out_dev
     g_ = _grid(grid)
     _check(_lib.rte_media_lognormal(C.byref(g_), float(dx_mm), C.c_uint64(int(seed)), float(mean), float(sigma_log),
                                     float(corr_len_mm), _dev(out_dev), _dev(scratch_dev), _stream_ptr(stream)))
+
+
+def rte_media_lognormal_noalloc(grid, dx_mm, seed, mean, sigma_log, corr_len_mm, out_dev, stream=None):
+    """Allocation-free variant (static in-library scratch, at most 2 097 152 cells; include/rte.h)."""
+    g_ = _grid(grid)
+    _check(_lib.rte_media_lognormal_noalloc(C.byref(g_), float(dx_mm), C.c_uint64(int(seed)), float(mean), float(sigma_log),
+                                            float(corr_len_mm), _dev(out_dev), _stream_ptr(stream)))
 
 
 def rte_pml_profile(grid, pml, mu_b_dev=None, inside_dev=None, stream=None):

@@ -1515,6 +1515,70 @@ int rte_media_lognormal(const rte_grid* grid, float dx, uint64_t seed, float mea
     return e == cudaSuccess ? RTE_OK : RTE_ECUDA;
 }
 
+// ---- allocation-free variant of the log-normal generator --------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (CUDA-graph capture, tight serving loops, harnesses that forbid it): the blur
+// scratch (one float per cell) and the two reduction doubles that rte_media_lognormal takes from the caller / from
+// cudaMalloc live in ONE file-scope device array of fixed size.  Every GPU that loads the library holds it until exit.
+constexpr long long kNoAllocMaxCells = 2097152;                      // 128^3 cells: 8 MiB of blur scratch
+constexpr size_t kNoAllocBytes = (size_t)kNoAllocMaxCells * sizeof(float) + 256;   // + one 256-byte slot for the moments
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: resolve it once per device, with
+// that device current, and hand the kernels the resolved pointer.
+static cudaError_t noalloc_scratch_address(unsigned char** ptr_out) {
+    static std::mutex mu;
+    static unsigned char* resolved[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!resolved[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        resolved[dev] = (unsigned char*)p;
+    }
+    *ptr_out = resolved[dev];
+    return cudaSuccess;
+}
+
+int rte_media_lognormal_noalloc(const rte_grid* grid, float dx, uint64_t seed, float mean, float sigma_log, float corr_len,
+                                float* out_dev, void* cuda_stream) {
+    if (!grid || (grid->dim != 2 && grid->dim != 3) || grid->nx < 1 || grid->ny < 1 || grid->nz < 1)
+        return fail(nullptr, RTE_EINVAL, "rte_media_lognormal_noalloc: bad grid");
+    if (!(dx > 0) || !(mean > 0) || !(sigma_log >= 0) || !(corr_len > 0) || !out_dev)
+        return fail(nullptr, RTE_EINVAL, "rte_media_lognormal_noalloc: bad argument");
+    const long long G = (long long)grid->nx * grid->ny * grid->nz;
+    if (G > kNoAllocMaxCells)
+        return fail(nullptr, RTE_EUNSUPPORTED, "rte_media_lognormal_noalloc: grid exceeds the static scratch (at most 2097152 cells = "
+                                               "128^3; use rte_media_lognormal with caller-owned scratch)");
+    unsigned char* base = nullptr;
+    const cudaError_t ea = noalloc_scratch_address(&base);
+    if (ea != cudaSuccess) return fail(nullptr, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(ea));
+    float* scratch = reinterpret_cast<float*>(base);
+    double* red = reinterpret_cast<double*>(base + (size_t)kNoAllocMaxCells * sizeof(float));
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int gb = grid_for(G, 256);
+    // the array keeps the last call's contents: the moments must start at zero (the blur scratch is fully overwritten)
+    if (cudaMemsetAsync(red, 0, 2 * sizeof(double), s) != cudaSuccess) return fail(nullptr, RTE_ECUDA, "CUDA: %s", "memset failed");
+    const float s_cells = corr_len / 1.41421356237f / dx;
+    const int R = (int)std::ceil(4.0f * s_cells);
+    const float inv2s2 = 1.0f / (2.0f * s_cells * s_cells);
+    k_white_noise<<<gb, 256, 0, s>>>(out_dev, G, (unsigned long long)seed);
+    float* a = out_dev;
+    float* b = scratch;
+    for (int axis = 0; axis < grid->dim; ++axis) {
+        k_blur_axis<<<gb, 256, 0, s>>>(b, a, grid->nx, grid->ny, grid->nz, axis, R, inv2s2);
+        float* t = a; a = b; b = t;
+    }
+    if (a != out_dev) cudaMemcpyAsync(out_dev, a, (size_t)G * sizeof(float), cudaMemcpyDeviceToDevice, s);
+    k_moments<<<gb, 256, 0, s>>>(out_dev, G, red);
+    k_lognormal_finish<<<gb, 256, 0, s>>>(out_dev, G, red, mean, sigma_log);
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? RTE_OK : fail(nullptr, RTE_ECUDA, "CUDA: %s", cudaGetErrorString(e));
+}
+
 int rte_pml_profile(const rte_grid* grid, const rte_pml* pml, float* mu_b_dev, unsigned char* inside_dev,
                     void* cuda_stream) {
     if (!grid || !pml || (grid->dim != 2 && grid->dim != 3) || grid->nx < 1 || grid->ny < 1 || grid->nz < 1) return RTE_EINVAL;
