@@ -358,9 +358,9 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {"cfg4": {0: 29696323999, 1: 43428465000, 2: 43432492000},       # profiles/r2j_summary.md §3 (ncu --set full,
-               "cfg3": {0: 4991200000, 1: 7194781000, 2: 7201715000},          # one launch per axis kernel)
-               "cfg2": {0: 246044416, 1: 344825344, 2: 345956864}}
+TRAFFIC_NCU = {"cfg4": {0: 29767685000, 1: 43429165000, 2: 43433319000},       # profiles/r2l_summary.md §3 (ncu --set full,
+               "cfg3": {0: 4989388000, 1: 7193650000, 2: 7201470000},          # one launch per axis kernel)
+               "cfg2": {0: 247507712, 1: 345311232, 2: 346320384}}
 
 
 def max_over_ranks(ms, dist, device):
