@@ -392,7 +392,7 @@ struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; };
 struct SpecRow { int n, P, TP, nt, TPx; };   // TP: pencils per y / z tile, TPx: per x tile
 constexpr SpecRow kSpec[] = {
     {384, 32, 1, 256, 1},   // cfg4: 384^3 P_7   (98 KB tile, 2 CTAs / SM)
-    {256, 18, 2, 288, 2},   // cfg3: 256^3 P_5   (288 B chunks = 9 whole sectors)
+    {256, 18, 2, 288, 1},   // cfg3: 256^3 P_5   (y/z: 288 B chunks = 9 whole sectors; x: one contiguous pencil per tile, 3 CTAs / SM)
     {128, 8, 4, 256, 4},    // cfg2: 128^3 P_3
     {512, 8, 2, 256, 2},    // cfg1: 512^2 P_7 (2-D)
     {64, 4, 8, 256, 8},     // cfg0: 64^2 P_3 (2-D)
@@ -508,7 +508,9 @@ cudaError_t launch_spec(int spec, const PassArgs& A, const LaunchPlan& L, cudaSt
     constexpr bool F = MODE == rtepass::MODE_FIRST;
     switch (spec) {
         case 0: return launch_one<24, 16, MODE, E, 32, 32, 256, 2, AX>(A, L, s);
-        case 1: return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3, AX>(A, L, s);
+        case 1:
+            if constexpr (AX == 0) return launch_one<16, 16, MODE, E, 18, 18, 288, 3, AX>(A, L, s);
+            else return launch_one<16, 16, MODE, E, 36, 18, 288, F ? 2 : 3, AX>(A, L, s);
         case 2: return launch_one<16, 8, MODE, E, 32, 8, 256, F ? 3 : 4, AX>(A, L, s);
         case 3: return launch_one<32, 16, MODE, E, 16, 8, 256, 2, AX>(A, L, s);
         case 4: return launch_one<8, 8, MODE, E, 32, 4, 256, 3, AX>(A, L, s);

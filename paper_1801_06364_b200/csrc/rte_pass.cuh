@@ -461,7 +461,12 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // ---- tail, specialised kernels: inverse first factor in registers, then one store / vector reduction per element ---------
 // (the coupling was applied in phase 1; every thread owns its column, so there is no barrier and no neighbour data)
 // FIRST: r holds the column's own psi (loaded by tail_load, the first task's before the phase-2 barrier).
-template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG, int AX>
+template <int N1, int N2, int QC, int PC, int AX>
+__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]);
+
+// LATE (FIRST instances whose register budget cannot hold the psi column next to the transform's): the re-read is issued
+// after the inverse DFT instead of before it; the higher occupancy of those instances hides its latency.
+template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG, int AX, bool LATE = false>
 __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile, const float* sig, long long base, int task,
                                           long long pencil0, float2 (&r)[N1]) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
@@ -476,6 +481,7 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
     if (MODE == MODE_FIRST) rtefft::dft_inv_swap<N1>(v);      // register pressure: see rte_fft.cuh
     else rtefft::dft_inv<N1>(v);
+    if (MODE == MODE_FIRST && LATE) tail_load<N1, N2, QC, PC, AX>(A, base, task, r);
     // x pass (AX == 0): the pencil is contiguous (cell stride 1, pencil stride n), so every address of the column is the
     // base plus a compile-time offset and folds into the instruction's immediate field
     float2* sp = AX == 0 ? A.acc + (base + (long long)t * n + b) * P + p
@@ -691,14 +697,15 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
         float2 r[N1];
         // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
         // phase 2 (the loads depend on nothing in shared memory)
-        if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC, AX>(A, base, tid, r);
+        constexpr bool LATE = MODE == MODE_FIRST && 65536 / ((NTC ? NTC : 1) * MINB) < 80;
+        if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX>(A, base, tid, r);
         __syncthreads();
-        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, tid, pencil0, r);
+        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            if (MODE == MODE_FIRST) tail_load<N1, N2, QC, PC, AX>(A, base, task, r2);
-            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX>(A, tile, sig, base, task, pencil0, r2);
+            if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX>(A, base, task, r2);
+            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();

@@ -205,10 +205,11 @@ inline int layout_tp(int dim, int N) {   // pencils per tile assumed by the mode
     return tp;
 }
 
-// pencils per x tile assumed by the model (= the specialised kernels' choice, rte_lib.cu kSpec TPx).  (One pencil per x tile
-// for the 18-pair records of P_5 — a contiguous, conflict-free tile — was measured 14 % slower on that pass: smaller
-// tiles, one task per thread.)
-inline int layout_tp_x(int dim, int N) { return layout_tp(dim, N); }
+// pencils per x tile assumed by the model (= the specialised kernels' choice, rte_lib.cu kSpec TPx).  The 18-pair records
+// of P_5 use ONE pencil per x tile: a contiguous tile whose own-element accesses are conflict-free (two stacked pencils
+// conflict at half of the row boundaries) and small enough for 3 CTAs per SM (measured: x pass -6 %; at 2 CTAs per SM
+// the same tile was 14 % slower).
+inline int layout_tp_x(int dim, int N) { return (dim == 3 && N == 5) ? 1 : layout_tp(dim, N); }
 
 // modelled wavefronts of ONE axis' gathers for a candidate layout
 inline int layout_cost_axis(int P, int TP, int axis, int E, const std::vector<int>& pos, const std::vector<int>& inv,
