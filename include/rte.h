@@ -162,7 +162,9 @@ int rte_set_extra_workspace(rte_ctx* ctx, void* extra_dev, size_t bytes);
  *     psi^{n+1} = E (psi^n - c dt T[psi^n]) + Phi c dt q(t_n),   E = exp(-c dt sigma_l),  Phi = (1 - E)/(c dt sigma_l).
  * A uniform field decays as exp(-c sigma_l t) with no O(dt) error, also in the PML, and the stiff diagonal
  * (c dt sigma_l > 2, where eq.(11) diverges) no longer bounds dt; the streaming bound (rte_stable_dt) is unchanged to
- * leading order.  Runs on the generic kernels.  Asynchronous on the stream. */
+ * leading order.  Grids with specialised kernels (the BASELINE configurations): the three specialised passes compute
+ * -c dt T, one pointwise kernel applies E, Phi and the source; every other grid: fused into the generic kernels.
+ * Asynchronous on the stream. */
 int rte_step_exp(rte_ctx* ctx, int nsteps);
 
 /* The time-independent transport operator of eq.(9): y = L x = T[x] + sigma_l x, so that eq.(9) reads

@@ -158,6 +158,40 @@ def test_exp_step_vs_oracle(shape, N, dt):
     assert abs(rte.rte_time_ps(ctx) - 6 * dt) < 1e-6
 
 
+@pytest.mark.parametrize("name", ["cfg2", "cfg0"])
+def test_exp_step_on_specialised_grids_vs_oracle(name):
+    """The grids of the BASELINE configurations take the two-kernel route of rte_step_exp (specialised passes for -c dt T,
+    then the pointwise exp / phi_1 / source kernel): cfg2 at full size with scalar media (uniform-g instance), PML and its
+    temporal-Gaussian source; cfg0's grid with a PML, maps and a constant source."""
+    if name == "cfg2":
+        cfg = wl.CONFIGS["cfg2"]
+        mu_a, mu_s, g = (float(v) for v in cfg.background)
+        src = wl.source_term(cfg)
+        src = dict(src, t0=2 * cfg.dt, sigma_t=1.5 * cfg.dt)
+        steps = 4
+    else:
+        cfg = wl.Config("cfg0pml", 2, 64, 64, 1, 3, 0.1, 0.002, 0.3, 12, (8, 0.01, 5.0), "random", "box", 0)
+        rng = np.random.default_rng(40)
+        mu_a = rng.uniform(0.01, 0.5, cfg.shape).astype(np.float32)
+        mu_s = rng.uniform(2.0, 20.0, cfg.shape).astype(np.float32)
+        g = rng.uniform(0.7, 0.95, cfg.shape).astype(np.float32)
+        src = dict(w=rng.standard_normal(cfg.C).astype(np.float32), S=rng.standard_normal((1, 7, 9)).astype(np.float32),
+                   origin=(5, 20, 0), extent=(9, 7, 1), kind=1, t0=0.0, sigma_t=1.0)      # the box reaches into the PML
+        steps = 12
+    psi0 = wl.random_state(cfg, seed=8)
+    ctx = gpu_create(cfg, mu_a, mu_s, g)
+    rte.rte_set_state(ctx, dev(psi0))
+    rte.rte_set_source(ctx, src["w"], dev(src["S"]), src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    o = make_oracle(cfg, mu_a, mu_s, g)
+    o.set_state(psi0)
+    o.set_source(src["w"], src["S"], src["origin"], src["extent"], src["kind"], src["t0"], src["sigma_t"])
+    l0 = rte.rte_launch_count(ctx)
+    rte.rte_step_exp(ctx, steps)
+    assert rte.rte_launch_count(ctx) - l0 == steps * (cfg.dim + 1)          # passes + the finish kernel: the two-kernel route
+    o.step_exp(steps)
+    assert_parity(gpu_state(ctx, cfg), o.get_state(), f"exp step on {name}'s grid")
+
+
 def test_exp_step_uniform_decay_exact_on_device():
     """P16 on the device: a uniform field decays as exp(-c sigma_l t) with no O(dt) error at c dt sigma_l ~ 1."""
     cfg = wl.Config("uni", 3, 16, 16, 16, 3, 0.1, 0.35, 0.3, 1, (0, 0.0, 0.0), "homogeneous", "none", 0)
