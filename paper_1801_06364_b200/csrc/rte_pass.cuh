@@ -391,7 +391,7 @@ constexpr int sig_pitch_l(int n, int TP) { return TP * (n + 2) + (36 - (TP * (n 
 template <int MAXC>
 struct SigCells { float sa[MAXC], ss[MAXC], g[MAXC]; };
 
-template <int N1, int N2, int MAXC>
+template <int N1, int N2, int MAXC, int AX>
 __device__ __forceinline__ void load_sig_cells(const PassArgs& A, SigCells<MAXC>& c, long long base, int valid, int tid, int nt) {
     constexpr int n = N1 * N2;
     const int ncell = n * A.TP;
@@ -402,7 +402,8 @@ __device__ __forceinline__ void load_sig_cells(const PassArgs& A, SigCells<MAXC>
         if (j < ncell) {
             const int t = j / n, i = j - t * n;
             if (t < valid) {
-                const long long cell = base + (long long)t * A.stride_t + (long long)i * A.stride_i;
+                // x pass: the tile's cells are contiguous (cell stride 1, pencil stride n)
+                const long long cell = AX == 0 ? base + j : base + (long long)t * A.stride_t + (long long)i * A.stride_i;
                 c.sa[k] = __ldg(A.sa + cell); c.ss[k] = __ldg(A.ss + cell);
                 if (!(A.g_uniform > 0.f)) c.g[k] = __ldg(A.gm + cell);
             }
@@ -672,14 +673,17 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
     __shared__ __align__(8) unsigned long long bar[N2];
     constexpr int NBAR = STACKED ? 1 : N2;
     const int tid = threadIdx.x, nt = NTC ? NTC : blockDim.x;
-    const int group = blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
-    const int valid = min(A.TP, A.pencils_per_group - tin * A.TP);
-    const long long base = group * A.group_stride + (long long)tin * A.TP * A.stride_t;
+    // specialised kernels: whole tiles only (the host checks pencils % TP == 0); their x pass has one group of contiguous pencils
+    constexpr int TPC = QC / (PC ? PC : 1);
+    const int group = (TMA && AX == 0) ? 0 : blockIdx.x / A.tiles_per_group, tin = blockIdx.x - group * A.tiles_per_group;
+    const int valid = TMA ? TPC : min(A.TP, A.pencils_per_group - tin * A.TP);
+    const long long base = (TMA && AX == 0) ? (long long)blockIdx.x * (TPC * n)
+                                            : group * A.group_stride + (long long)tin * A.TP * A.stride_t;
     const long long pencil0 = (long long)blockIdx.x * A.TP;
     if constexpr (TMA) {
         constexpr int MAXC = (n * (QC / (PC ? PC : 1)) + (NTC ? NTC : 1) - 1) / (NTC ? NTC : 1);
         SigCells<MAXC> cells;
-        if (MODE == MODE_FIRST) load_sig_cells<N1, N2, MAXC>(A, cells, base, valid, tid, nt);   // in flight during the TMA issue
+        if (MODE == MODE_FIRST) load_sig_cells<N1, N2, MAXC, AX>(A, cells, base, valid, tid, nt);   // in flight during the TMA issue
         if (tid < NBAR) {
             mbar_init(&bar[tid], 1);
             mbar_arrive_expect_tx(&bar[tid], (unsigned)(n / NBAR) * QC * 8u);
