@@ -617,47 +617,58 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
 //   new = E (psi + acc) + Phi c dt f(t_n) q,   E = exp(-c dt sigma_l),  Phi = (1 - E)/(c dt sigma_l)
 // in one pointwise kernel (in place on acc).  8 S + 3 S of traffic instead of the generic kernels' 8 S, but at the specialised
 // kernels' speed (cfg4: 31 instead of 53 ms per step).
-__global__ void k_exp_finish(float2* __restrict__ acc, const float2* __restrict__ psi, const float* __restrict__ sa,
-                             const float* __restrict__ ss, const float* __restrict__ gm, const int* __restrict__ deg,
-                             const float* __restrict__ srcS, const float* __restrict__ srcw, int ox, int oy, int oz, int ex,
-                             int ey, int ez, int nx, int ny, long long G, int P, float cdt, float amp) {
-    const long long total = G * P;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    const long long stride_cells = stride / P;
-    const int stride_p = (int)(stride - stride_cells * P);
-    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    long long cell = i / P;                                   // (cell, pair) advance incrementally: no division in the loop
-    int p = (int)(i - cell * P);
-    // cells of the source box lie in [box_lo, box_hi]: one comparison rejects almost every cell
+constexpr int kExpChunk = 64;      // cells per block round of k_exp_finish
+constexpr int kExpMaxDeg = 32;     // N + 1 <= 32
+
+__global__ void __launch_bounds__(256) k_exp_finish(float2* __restrict__ acc, const float2* __restrict__ psi,
+                                                    const float* __restrict__ sa, const float* __restrict__ ss,
+                                                    const float* __restrict__ gm, const int* __restrict__ deg,
+                                                    const float* __restrict__ srcS, const float* __restrict__ srcw, int ox, int oy,
+                                                    int oz, int ex, int ey, int ez, int nx, int ny, long long G, int P, int nsig,
+                                                    float cdt, float amp) {
+    // per chunk of cells: first the (cell, degree) table of c dt sigma_l and E = exp(-c dt sigma_l) in shared memory (one expf per
+    // cell and degree instead of two per element), then a coalesced sweep over the chunk's elements
+    __shared__ float tE[kExpChunk * kExpMaxDeg], tA[kExpChunk * kExpMaxDeg];
     const long long box_lo = ((long long)oz * ny + oy) * nx + ox;
     const long long box_hi = ((long long)(oz + ez - 1) * ny + (oy + ey - 1)) * nx + (ox + ex - 1);
-    for (; i < total; i += stride) {
-        const float a0 = __ldg(sa + cell), s0 = __ldg(ss + cell), g = __ldg(gm + cell);
-        float e[2], arg[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
+    const long long nchunks = (G + kExpChunk - 1) / kExpChunk;
+    for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+        const long long cell0 = ch * kExpChunk;
+        const int ncell = (int)min((long long)kExpChunk, G - cell0);
+        __syncthreads();                                       // the previous chunk's table is no longer read
+        for (int j = threadIdx.x; j < ncell * nsig; j += blockDim.x) {
+            const int c = j / nsig, l = j - c * nsig;
+            const float g = __ldg(gm + cell0 + c);
             float pw = 1.f;
-            for (int l = __ldg(deg + 2 * p + h); l > 0; --l) pw *= g;             // g^l by repeated multiplication (R16)
-            arg[h] = cdt * fmaf(s0, 1.f - pw, a0);                                // c dt sigma_l
-            e[h] = expf(-arg[h]);
+            for (int k = 0; k < l; ++k) pw *= g;               // g^l by repeated multiplication (R16)
+            const float a = cdt * fmaf(__ldg(ss + cell0 + c), 1.f - pw, __ldg(sa + cell0 + c));   // c dt sigma_l
+            tA[j] = a;
+            tE[j] = expf(-a);
         }
-        const float2 u = __ldg(psi + i), t = acc[i];
-        float2 r = make_float2(e[0] * (u.x + t.x), e[1] * (u.y + t.y));
-        if (amp != 0.f && cell >= box_lo && cell <= box_hi) {
-            const int x = (int)(cell % nx);
-            const long long rr = cell / nx;
-            const int bx = x - ox, by = (int)(rr % ny) - oy, bz = (int)(rr / ny) - oz;
-            if (bx >= 0 && bx < ex && by >= 0 && by < ey && bz >= 0 && bz < ez) {
-                const float q = amp * __ldg(srcS + ((size_t)bz * ey + by) * ex + bx);
-                const float ph0 = arg[0] > 0.f ? -expm1f(-arg[0]) / arg[0] : 1.f;   // phi_1
-                const float ph1 = arg[1] > 0.f ? -expm1f(-arg[1]) / arg[1] : 1.f;
-                r.x = fmaf(ph0 * __ldg(srcw + 2 * p), q, r.x);
-                r.y = fmaf(ph1 * __ldg(srcw + 2 * p + 1), q, r.y);
+        __syncthreads();
+        const long long i0 = cell0 * P;
+        for (int j = threadIdx.x; j < ncell * P; j += blockDim.x) {
+            const int c = j / P, p = j - c * P;
+            const int l0 = __ldg(deg + 2 * p), l1 = __ldg(deg + 2 * p + 1);
+            const float e0 = tE[c * nsig + l0], e1 = tE[c * nsig + l1];
+            const float2 u = __ldg(psi + i0 + j), t = acc[i0 + j];
+            float2 r = make_float2(e0 * (u.x + t.x), e1 * (u.y + t.y));
+            const long long cell = cell0 + c;
+            if (amp != 0.f && cell >= box_lo && cell <= box_hi) {
+                const int x = (int)(cell % nx);
+                const long long rr = cell / nx;
+                const int bx = x - ox, by = (int)(rr % ny) - oy, bz = (int)(rr / ny) - oz;
+                if (bx >= 0 && bx < ex && by >= 0 && by < ey && bz >= 0 && bz < ez) {
+                    const float q = amp * __ldg(srcS + ((size_t)bz * ey + by) * ex + bx);
+                    const float a0 = tA[c * nsig + l0], a1 = tA[c * nsig + l1];
+                    const float ph0 = a0 > 0.f ? -expm1f(-a0) / a0 : 1.f;   // phi_1
+                    const float ph1 = a1 > 0.f ? -expm1f(-a1) / a1 : 1.f;
+                    r.x = fmaf(ph0 * __ldg(srcw + 2 * p), q, r.x);
+                    r.y = fmaf(ph1 * __ldg(srcw + 2 * p + 1), q, r.y);
+                }
             }
+            acc[i0 + j] = r;
         }
-        acc[i] = r;
-        p += stride_p; cell += stride_cells;
-        if (p >= P) { p -= P; ++cell; }
     }
 }
 
@@ -676,9 +687,9 @@ int one_step(rte_ctx* c, cudaEvent_t* ev = nullptr, PassKind kind = KIND_STEP, c
         const int rc = euler_update(c, c->psi, c->part, tn, KIND_STREAM, ev);
         if (rc != RTE_OK) return rc;
         const float amp = c->src_kind != 0 ? (float)((double)c->c * (double)c->dt * source_time_factor(c, tn)) : 0.f;
-        k_exp_finish<<<grid_for(c->G * c->P, 256), 256, 0, c->stream>>>(c->part, c->psi, c->sa, c->ss, c->gm, c->deg, c->srcS, c->srcw,
-            c->src_org[0], c->src_org[1], c->src_org[2], c->src_ext[0], c->src_ext[1], c->src_ext[2], c->grid.nx, c->grid.ny,
-            c->G, c->P, c->c * c->dt, amp);
+        k_exp_finish<<<grid_for((c->G + kExpChunk - 1) / kExpChunk, 1), 256, 0, c->stream>>>(c->part, c->psi, c->sa, c->ss, c->gm,
+            c->deg, c->srcS, c->srcw, c->src_org[0], c->src_org[1], c->src_org[2], c->src_ext[0], c->src_ext[1], c->src_ext[2],
+            c->grid.nx, c->grid.ny, c->G, c->P, c->N + 1, c->c * c->dt, amp);
         c->launches += 1;
         if (cudaGetLastError() != cudaSuccess) return fail(c, RTE_ECUDA, "CUDA: %s", "exp finish launch failed");
     } else {
