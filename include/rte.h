@@ -215,6 +215,13 @@ int rte_fluence_host(rte_ctx* ctx, float* phi_host); /* device -> host, synchron
  * the steady-state test of configs[3] (R17).  Synchronises the stream. */
 int rte_fluence_change(rte_ctx* ctx, double* rel_change_out);
 
+/* Instability / NaN guard (R10; the step itself never checks its time step, as in the paper):
+ * energy_out = sum_c w_l ||psi_c||_2^2 over the whole grid with w_l = 2l+1 (3-D) or 1 (m = 0), 2 (m >= 1) (2-D) — the norm in
+ * which the streaming operator is skew-adjoint, so in source-free stretches a stable run never lets it grow — and
+ * nonfinite_out = the number of NaN / Inf values in the state (they are left out of the sum).  Either may be NULL.
+ * Synchronises the stream. */
+int rte_energy(rte_ctx* ctx, double* energy_out, long long* nonfinite_out);
+
 int rte_time_ps(const rte_ctx* ctx, double* t_out);  /* t = steps taken since the last reset * dt */
 int rte_sync(rte_ctx* ctx);                          /* stream synchronise; surfaces deferred CUDA errors */
 const char* rte_last_error(const rte_ctx* ctx);      /* ctx may be NULL: text of the last failed rte_create */

@@ -67,6 +67,7 @@ _lib.rte_solve_steady.argtypes = [_vp, _i, C.c_double, _i, _i, _f, C.POINTER(_i)
 _lib.rte_step_profile.argtypes = [_vp, _i, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
 _lib.rte_fluence_change.argtypes = [_vp, C.POINTER(C.c_double)]
 _lib.rte_time_ps.argtypes = [_vp, C.POINTER(C.c_double)]
+_lib.rte_energy.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
 _lib.rte_sync.argtypes = [_vp]
 _lib.rte_last_error.argtypes = [_vp]
 _lib.rte_last_error.restype = C.c_char_p
@@ -82,7 +83,7 @@ EXPORTED = ["rte_num_coeffs", "rte_coupling_table", "rte_storage_layout", "rte_w
             "rte_set_source", "rte_set_source_host", "rte_step", "rte_step_ssprk3", "rte_step_exp", "rte_step_profile",
             "rte_extra_workspace_bytes", "rte_set_extra_workspace", "rte_stable_dt", "rte_apply_operator",
             "rte_solve_steady", "rte_fluence", "rte_fluence_host",
-            "rte_fluence_change", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
+            "rte_fluence_change", "rte_energy", "rte_time_ps", "rte_sync", "rte_last_error", "rte_launch_count",
             "rte_media_ellipsoids", "rte_media_lognormal", "rte_media_lognormal_noalloc", "rte_pml_profile"]
 
 
@@ -331,6 +332,13 @@ def rte_fluence_change(ctx):
     out = C.c_double(0)
     _check(_lib.rte_fluence_change(ctx.handle, C.byref(out)), ctx.handle)
     return float(out.value)
+
+
+def rte_energy(ctx):
+    """(weighted energy sum_c w_l ||psi_c||^2, number of non-finite state values) — the instability guard of include/rte.h."""
+    e, n = C.c_double(0), C.c_longlong(0)
+    _check(_lib.rte_energy(ctx.handle, C.byref(e), C.byref(n)), ctx.handle)
+    return float(e.value), int(n.value)
 
 
 def rte_time_ps(ctx):

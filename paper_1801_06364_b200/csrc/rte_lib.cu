@@ -280,6 +280,28 @@ __global__ void k_fluence_change(const float* __restrict__ psi, float* __restric
     if ((threadIdx.x & 31) == 0) { atomicAdd(&red[0], d2); atomicAdd(&red[1], n2); }
 }
 
+// weighted energy  sum_c (2l+1) ||psi_c||^2  (2-D: weight 1 for m = 0, 2 for m >= 1) and the number of non-finite values:
+// the instability guard of reading R10 (forward Euler beyond its bound makes this grow in source-free stretches)
+__global__ void k_energy(const float* __restrict__ psi, const int* __restrict__ deg, const int* __restrict__ ext_of_slot,
+                         long long G, int Cp, int dim, double* __restrict__ red) {
+    double e = 0, bad = 0;
+    const long long total = G * Cp;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int s = (int)(i % Cp);
+        if (ext_of_slot[s] < 0) continue;                       // pad slot
+        const float v = psi[i];
+        if (!isfinite(v)) { bad += 1.0; continue; }
+        const int l = deg[s];
+        const double w = dim == 3 ? (double)(2 * l + 1) : (l == 0 ? 1.0 : 2.0);
+        e += w * (double)v * (double)v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        e += __shfl_down_sync(0xffffffffu, e, o);
+        bad += __shfl_down_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&red[0], e); atomicAdd(&red[1], bad); }
+}
+
 // ---- geometry generators -------------------------------------------------------------------------------------------
 __global__ void k_ellipsoids(float* __restrict__ mu_a, float* __restrict__ mu_s, float* __restrict__ g,
                              const float* __restrict__ ell, int n_ell, float bg_a, float bg_s, float bg_g, int dim,
@@ -1495,6 +1517,22 @@ int rte_fluence_host(rte_ctx* ctx, float* phi_host) {
     if (rc != RTE_OK) return rc;
     CUDA_TRY(ctx, cudaMemcpyAsync(phi_host, ctx->part, (size_t)ctx->G * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
     CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    return RTE_OK;
+}
+
+int rte_energy(rte_ctx* ctx, double* energy_out, long long* nonfinite_out) {
+    if (!ctx) return RTE_ESTATE;
+    if (!energy_out && !nonfinite_out) return fail(ctx, RTE_EINVAL, "null output pointers");
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->red, 0, 2 * sizeof(double), ctx->stream));
+    k_energy<<<grid_for(ctx->G * ctx->Cp, 256), 256, 0, ctx->stream>>>((const float*)ctx->psi, ctx->deg, ctx->ext_of_slot, ctx->G,
+                                                                    ctx->Cp, ctx->grid.dim, ctx->red);
+    ctx->launches += 1;
+    CUDA_TRY(ctx, cudaGetLastError());
+    double h[2] = {0, 0};
+    CUDA_TRY(ctx, cudaMemcpyAsync(h, ctx->red, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (energy_out) *energy_out = h[0];
+    if (nonfinite_out) *nonfinite_out = (long long)h[1];
     return RTE_OK;
 }
 

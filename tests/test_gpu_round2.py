@@ -304,3 +304,42 @@ def test_solve_steady_2d_vs_oracle():
     _, orr = o.solve_steady(restart=40, tol=1e-10, max_restarts=200)
     assert orr <= 1e-10 and rr <= 2e-6, (rr, orr)
     assert_parity(gpu_state(ctx, cfg), o.get_state(), f"2-D steady ({napp} sweeps)")
+
+
+# ---- instability / NaN guard --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dim", [3, 2])
+def test_energy_guard(dim):
+    """rte_energy = sum_c w_l ||psi_c||^2 (w = 2l+1 in 3-D; 1, 2, 2, ... in 2-D) against numpy; it never grows in a source-free
+    run at the dt recommended by rte_stable_dt and blows up at 4x the bound (reading R10); NaNs are counted, not summed."""
+    n, N, dx, c = 32, 3, 0.2, 0.3
+    med = (0.02, 4.0, 0.8)
+    nz = n if dim == 3 else 1
+    bound, dt_ok = rte.rte_stable_dt(dim, N, n, dx, c, *med)
+    cfg = wl.Config("e", dim, n, n, nz, N, dx, dt_ok, c, 0, (0, 0.0, 0.0), "homogeneous", "none", 0)
+    psi0 = wl.random_state(cfg, seed=9, decay=1.0)          # white in space and degree: every mode up to the corner Nyquist
+    L = np.array([int(np.floor(np.sqrt(i))) for i in range(cfg.C)]) if dim == 3 else np.array([0] + [m for m in range(1, N + 1) for _ in range(2)])
+    w = (2 * L + 1) if dim == 3 else np.where(L == 0, 1.0, 2.0)
+    ctx = rte.rte_create(cfg.grid, N, dx, dt_ok, c, *med)
+    rte.rte_set_state(ctx, dev(psi0))
+    e0, bad = rte.rte_energy(ctx)
+    ref = float((w[:, None, None, None] * psi0.astype(np.float64) ** 2).sum())
+    assert bad == 0 and abs(e0 / ref - 1) < 1e-6
+    prev = e0
+    for _ in range(8):
+        rte.rte_step(ctx, 25)
+        e, bad = rte.rte_energy(ctx)
+        assert bad == 0 and e <= prev * (1 + 1e-6)
+        prev = e
+    # 4x the bound: the corner modes are amplified every step
+    ctx2 = rte.rte_create(cfg.grid, N, dx, 4.0 * bound, c, *med)
+    rte.rte_set_state(ctx2, dev(psi0))
+    rte.rte_step(ctx2, 200)
+    e2, _ = rte.rte_energy(ctx2)
+    assert e2 > 10 * e0
+    # NaNs / Infs are counted and kept out of the sum
+    bad_state = psi0.copy()
+    bad_state[1, 0, 3, 4] = np.nan
+    bad_state[2, 0, 5, 6] = np.inf
+    rte.rte_set_state(ctx, dev(bad_state))
+    e3, bad3 = rte.rte_energy(ctx)
+    assert bad3 == 2 and np.isfinite(e3) and e3 < e0
