@@ -1314,8 +1314,18 @@ __global__ void k_source_field(float* __restrict__ b, const float* __restrict__ 
     }
 }
 
+static int solve_steady_impl(rte_ctx* ctx, int restart, double tol, int max_restarts, int precond_steps, float precond_dt_ps,
+                             int* applications_out, double* relres_out);
+
 int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, int precond_steps, float precond_dt_ps,
                      int* applications_out, double* relres_out) {
+    return guarded([&]() -> int {     // the preconditioner's tables are built in host vectors: nothing may throw across the ABI
+        return solve_steady_impl(ctx, restart, tol, max_restarts, precond_steps, precond_dt_ps, applications_out, relres_out);
+    });
+}
+
+static int solve_steady_impl(rte_ctx* ctx, int restart, double tol, int max_restarts, int precond_steps, float precond_dt_ps,
+                             int* applications_out, double* relres_out) {
     using namespace rtesolve;
     if (!ctx) return RTE_ESTATE;
     if (restart < 1 || restart > kMaxRestart || !(tol > 0) || max_restarts < 0 || precond_steps < 0 ||
