@@ -6,6 +6,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
@@ -66,6 +67,7 @@ struct rte_ctx {
     float* srcw = nullptr;
     float* srcS = nullptr;
     size_t srcS_cap = 0;
+    int tuned_nt[3] = {0, 0, 0};   // generic kernels: block size per axis measured at the first sweep (0: not yet)
     int first_axis = 0;            // axis of the FIRST pass (the one that stores; the others accumulate): x
     float g_uniform = 0.f;         // > 0: the anisotropy g is one number (media.g_is_map == 0): kernels use the 2-number table
     char* extra = nullptr;         // caller-owned extra workspace (rte_set_extra_workspace): state-sized fields for
@@ -410,7 +412,7 @@ int check_grid(const rte_grid* g) {
 // ---------------------------------------------------------------------------------------------------------------------
 // A pass runs either a kernel specialised at compile time for (n, P, TP, block size) — the five BASELINE.json
 // configurations — or the generic kernel (run-time P, TP, block size, FIRST/ACC) for every other supported extent / order.
-struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; };
+struct LaunchPlan { int TP, nt, blocks, spec; size_t smem; int ncand; int cand[16]; };   // cand: block sizes worth timing (generic)
 
 struct SpecRow { int n, P, TP, nt, TPx; };   // TP: pencils per y / z tile, TPx: per x tile
 constexpr SpecRow kSpec[] = {
@@ -429,6 +431,8 @@ size_t pass_smem(int n, int Q, int TP, int nsig, bool diag) {
 }
 
 constexpr size_t kMaxSmem = 226 * 1024;   // 227 KB per CTA minus the static mbarrier slot
+
+int generic_kernel_regs(int n);      // registers per thread of the generic instance for pencil length n (defined below)
 
 LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     const int first_axis = c->first_axis;
@@ -459,17 +463,29 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
         while (tp * P < 32 && tp < 8) tp *= 2;
         while (tp > 1 && pass_smem(n, tp * P, tp, c->N + 1, diag) > 100 * 1024) tp /= 2;
         while (tp > 1 && tp > A.pencils_per_group) tp /= 2;
+        // block size by modelled throughput: the share of useful lanes in the two task loops (Q*N2 and Q*N1 tasks) times
+        // the occupancy it allows (CTAs per SM by shared memory, registers of this instance and threads; 24 warps per SM
+        // count as saturated).  (The first version minimised idle lanes only and picked e.g. 64-thread blocks — 6 warps per
+        // SM — for 192^3 P_5.)
         const int Q = tp * P;
         const int T1 = Q * T.N2, T2 = Q * T.N1;
-        int best = 128; double best_cost = 1e30;
+        const size_t smem = pass_smem(n, Q, tp, c->N + 1, diag) + 1024;       // + the per-CTA reservation
+        const int regs = (generic_kernel_regs(n) + 7) / 8 * 8;
+        int best = 128; double best_score = -1.0;
         const int ntmax = rtepass::generic_max_threads(T.N1, T.N2);   // by register need of the transforms (rte_pass.cuh)
         for (int nt = 64; nt <= ntmax; nt += 32) {
             if (nt > T1 && nt > T2 && nt > 64) break;
-            const double w1 = (double)((T1 + nt - 1) / nt * nt - T1) / T1, w2 = (double)((T2 + nt - 1) / nt * nt - T2) / T2;
-            const double cost = w1 + w2;
-            if (cost <= best_cost + 1e-12) { best_cost = cost; best = nt; }
+            const double useful = (double)(T1 + T2) / (double)((T1 + nt - 1) / nt * nt + (T2 + nt - 1) / nt * nt);
+            int ctas = (int)((size_t)228 * 1024 / smem);
+            if (regs > 0) ctas = std::min(ctas, 65536 / (regs * nt));
+            ctas = std::min(std::min(ctas, 2048 / nt), 32);
+            if (ctas < 1) ctas = 1;
+            const double warps = std::min(24.0, (double)ctas * nt / 32.0);
+            const double score = useful * warps / 24.0;
+            if (score >= best_score - 1e-12) { best_score = score; best = nt; }
+            if (useful >= 0.74 && L.ncand < 16) L.cand[L.ncand++] = nt;
         }
-        L.TP = tp; L.nt = best;
+        L.TP = tp; L.nt = c->tuned_nt[axis] > 0 ? c->tuned_nt[axis] : best;
     }
     A.TP = L.TP;
     A.tiles_per_group = (A.pencils_per_group + L.TP - 1) / L.TP;
@@ -520,6 +536,24 @@ cudaError_t launch_generic(int n, const PassArgs& A, const LaunchPlan& L, cudaSt
     RTE_SPLITS(RTE_GENERIC_CASE)
 #undef RTE_GENERIC_CASE
     return cudaErrorInvalidValue;
+}
+
+int generic_kernel_regs(int n) {
+    static std::mutex mu;
+    static int cache[1025] = {};
+    if (n < 0 || n > 1024) return 0;
+    std::lock_guard<std::mutex> lock(mu);
+    if (cache[n] == 0) {
+        cudaFuncAttributes at{};
+        cudaError_t e = cudaErrorInvalidValue;
+#define RTE_GENERIC_REGS(N1_, N2_) \
+        if (n == (N1_) * (N2_)) e = cudaFuncGetAttributes(&at, rtepass::pass_kernel<N1_, N2_, rtepass::MODE_RT, 4, 0, 0, 0, 1, false, 0>);
+        RTE_SPLITS(RTE_GENERIC_REGS)
+#undef RTE_GENERIC_REGS
+        cache[n] = e == cudaSuccess ? at.numRegs : -1;
+        if (e != cudaSuccess) cudaGetLastError();
+    }
+    return cache[n] > 0 ? cache[n] : 0;
 }
 
 // E = 2 on the z axis of 3-D runs (fan-in of the z coupling is at most 2 pairs, rte_tables.h), 4 otherwise.
@@ -594,8 +628,7 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
     const int fa = c->first_axis;
     // the FIRST pass stores, the others add to what it stored: it goes first
     int order[3] = {fa, fa == 0 ? 1 : 0, fa == 2 ? 1 : 2};
-    for (int k = 0; k < naxes; ++k) {
-        const int axis = order[k];
+    auto launch_axis = [&](int axis, int nt_override) -> cudaError_t {
         PassArgs A{};
         A.psi = in; A.acc = out;
         A.cpl = kind == KIND_OPER ? c->ax[axis].cpl_op : (kind == KIND_ALT ? c->ax[axis].cpl_alt : c->ax[axis].cpl);
@@ -612,7 +645,8 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
         for (int j = 0; j < 3; ++j) { A.src_org[j] = c->src_org[j]; A.src_ext[j] = c->src_ext[j]; }
         A.src_amp = 0.f; A.src_amp_dev = nullptr;
         A.nx = c->grid.nx; A.ny = c->grid.ny;
-        const LaunchPlan L = plan_pass(c, axis, A, kind);
+        LaunchPlan L = plan_pass(c, axis, A, kind);
+        if (nt_override > 0) L.nt = nt_override;
         const int n = c->ax[axis].n;
         if (A.first && c->src_kind != 0 && kind == KIND_ALT) {
             A.src_amp = c->c * c->dt_alt * c->alt_src;
@@ -621,13 +655,57 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
             A.src_amp_dev = amp_dev;
             if (amp_dev) A.src_amp = 1.f;      // non-zero: the kernel reads the device value
         }
-        cudaError_t e;
         using namespace rtepass;
-        if (L.spec < 0) e = launch_generic(n, A, L, c->stream);
-        else if (axis == 0) e = launch_spec<MODE_FIRST, 4, 0>(L.spec, A, L, c->stream);
-        else if (axis == 1) e = launch_spec<MODE_ACC, 4, 1>(L.spec, A, L, c->stream);
+        if (L.spec < 0) return launch_generic(n, A, L, c->stream);
+        if (axis == 0) return launch_spec<MODE_FIRST, 4, 0>(L.spec, A, L, c->stream);
+        if (axis == 1) return launch_spec<MODE_ACC, 4, 1>(L.spec, A, L, c->stream);
         // z axis: coupling fan-in 2 (rte_tables.h); plan_pass falls back to the generic kernel otherwise
-        else e = launch_spec<MODE_ACC, 2, 2>(L.spec, A, L, c->stream);
+        return launch_spec<MODE_ACC, 2, 2>(L.spec, A, L, c->stream);
+    };
+    // Generic kernels: the block size of every axis is MEASURED once per context, at its first sweep, among the candidates the
+    // occupancy model leaves (the model alone mispredicts by up to 30 %): each candidate is launched twice on the buffers of
+    // this sweep and the second launch is timed.  `out` only holds garbage afterwards, and the FIRST pass of the real sweep
+    // below overwrites all of it.  Results do not depend on the block size.  Skipped under stream capture.  One stream
+    // synchronisation per context.
+    {
+        bool need = false;
+        for (int axis = 0; axis < naxes; ++axis) {
+            PassArgs A{};
+            if (c->tuned_nt[axis] == 0 && plan_pass(c, axis, A, kind).spec < 0) need = true;
+        }
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (need && halt == nullptr && cudaStreamIsCapturing(c->stream, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusNone) {
+            cudaEvent_t e0 = nullptr, e1 = nullptr;
+            if (cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess) {
+                for (int axis = 0; axis < naxes; ++axis) {
+                    PassArgs A{};
+                    const LaunchPlan L = plan_pass(c, axis, A, kind);
+                    if (c->tuned_nt[axis] != 0 || L.spec >= 0) continue;
+                    float best_ms = 1e30f;
+                    int best_nt = L.nt;
+                    for (int k = 0; k < L.ncand; ++k) {
+                        if (launch_axis(axis, L.cand[k]) != cudaSuccess) { cudaGetLastError(); continue; }
+                        cudaEventRecord(e0, c->stream);
+                        const cudaError_t le = launch_axis(axis, L.cand[k]);
+                        cudaEventRecord(e1, c->stream);
+                        c->launches += 2;
+                        float ms = 0.f;
+                        if (le != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) {
+                            cudaGetLastError();
+                            continue;
+                        }
+                        if (ms < best_ms) { best_ms = ms; best_nt = L.cand[k]; }
+                    }
+                    c->tuned_nt[axis] = best_nt;
+                }
+            }
+            if (e0) cudaEventDestroy(e0);
+            if (e1) cudaEventDestroy(e1);
+        }
+    }
+    for (int k = 0; k < naxes; ++k) {
+        const int axis = order[k];
+        const cudaError_t e = launch_axis(axis, 0);
         if (e != cudaSuccess) return fail(c, RTE_ECUDA, "pass launch: %s", cudaGetErrorString(e));
         c->launches += 1;
         if (ev) cudaEventRecord(ev[k], c->stream);
