@@ -418,7 +418,11 @@ def steady_state_run(rte, wl, cfg, torch, dev, max_steps=20000, tol=1e-6, plain_
     del ctx0
     torch.cuda.empty_cache()
     dtp = 0.3 * cfg.dx / cfg.c
-    variants = [("gmres20_rk3x8", dict(restart=20, tol=1e-5, max_restarts=100, precond_steps=8, precond_dt_ps=dtp))]
+    # restart 40 needs 46 state-sized fields of extra workspace (cfg3: 111 GB); smaller boards: restart 20 (26 fields, ~20 % slower)
+    free_b, _ = torch.cuda.mem_get_info()
+    field_b = 4 * cfg.G * (cfg.C + cfg.C % 2)
+    restart = 40 if free_b > 50 * field_b else 20
+    variants = [(f"gmres{restart}_rk3x8", dict(restart=restart, tol=1e-5, max_restarts=100, precond_steps=8, precond_dt_ps=dtp))]
     if plain_krylov:
         variants.append(("gmres30_plain", dict(restart=30, tol=1e-5, max_restarts=400)))
     for name, kw in variants:
