@@ -357,9 +357,9 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {"cfg4": {0: 29837960000, 1: 43430859000, 2: 43431673000},       # profiles/r2n_summary.md §3 (ncu --set full,
-               "cfg3": {0: 5008276000, 1: 7193785000, 2: 7201139000},          # one launch per axis kernel)
-               "cfg2": {0: 246656255, 1: 346291200, 2: 346157056}}
+TRAFFIC_NCU = {"cfg4": {0: 29832065999, 1: 43429994000, 2: 43433243000},       # profiles/r2p_summary.md §3 (ncu --set full,
+               "cfg3": {0: 5008290000, 1: 7193856999, 2: 7205445000},          # one launch per axis kernel)
+               "cfg2": {0: 247262975, 1: 345633536, 2: 347201024}}
 
 
 def max_over_ranks(ms, dist, device):
