@@ -1259,6 +1259,7 @@ int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, 
 // SAME launch code and replayed; the time-dependent source amplitude c dt f(t_n) of every captured step is read by
 // the x kernel from a small device table that the host refreshes, stream-ordered, before each replay.
 constexpr int kGraphSteps = 32;
+constexpr int kGraphBuildMin = 4;     // calls of fewer steps never pay for a capture
 constexpr size_t kGraphMaxStateBytes = (size_t)24 << 20;   // states up to 24 MB (cfg1: 16.8 MB) are L2-resident
 
 int build_graph(rte_ctx* c) {
@@ -1293,7 +1294,9 @@ int rte_step(rte_ctx* ctx, int nsteps) {
     return guarded([&]() -> int {
         int left = nsteps;
         const bool small = (size_t)ctx->G * ctx->Cp * sizeof(float) <= kGraphMaxStateBytes;
-        if (small && left >= kGraphSteps + 1) {
+        // the graph is captured and instantiated (~1 ms) as soon as a call asks for a handful of steps — e.g. a warm-up —
+        // so that it is ready when a long run follows; it is replayed only when a whole 32-step batch is left
+        if (small && left >= kGraphBuildMin) {
             if (ctx->launches_warm == 0) {                  // one eager step first: per-device kernel attributes get set
                 const int rc = one_step(ctx);
                 if (rc != RTE_OK) return rc;
