@@ -198,8 +198,9 @@ int rte_solve_steady(rte_ctx* ctx, int restart, double tol, int max_restarts, in
  * (Shu-Osher form) built from the same Euler update E(u; t) = u + dt F(u, t) of eq.(9):
  *   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2).
  * Its stability region contains the imaginary axis up to sqrt(3), so dt may approach dx/c instead of the
- * scattering-limited Euler bound (R10).  Three Euler updates (9 pass kernels in 3-D) and two state-wide
- * axpby kernels per step.  Needs 1 field of extra workspace (rte_set_extra_workspace), RTE_EINVAL without it.
+ * scattering-limited Euler bound (R10).  Three Euler updates (9 pass kernels in 3-D); the two convex combinations
+ * are fused into them (the tables of stages 2 and 3 carry the factors 1/4 and 2/3, their first pass adds 3/4 and 1/3 of u^n
+ * while it stores).  Needs 1 field of extra workspace (rte_set_extra_workspace), RTE_EINVAL without it.
  * Asynchronous on the stream; rte_time_ps advances by dt per step. */
 int rte_step_ssprk3(rte_ctx* ctx, int nsteps);
 

@@ -34,6 +34,8 @@ struct AxisTables {
     CplEntry* cpl = nullptr;      // weights x (-c dt) (2 pi / (n dx)) / n : the time step (eq.(11))
     CplEntry* cpl_op = nullptr;   // weights x (+1)    (2 pi / (n dx)) / n : the steady-state operator L = T + sigma_l
     CplEntry* cpl_alt = nullptr;  // weights x (-c dt_alt) ... : Euler updates with another time step (solver preconditioner)
+    CplEntry* cpl_rk[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [dt | dt_alt][x 1/4 | x 2/3]: the scaled Euler
+                                  // updates of the SSP-RK3 stages (the stage combination is fused into the passes)
     float2* tw = nullptr;         // forward twiddles of this axis (generic kernels)
     int n = 0, N1 = 0, N2 = 0, maxcnt = 0, npure = 0;   // npure: leading coupling slots with pure blocks (rte_tables.h)
 };
@@ -495,9 +497,9 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     return L;
 }
 
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, bool BASE = false>
 cudaError_t launch_one_impl(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
-    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG, AX>;
+    auto kern = rtepass::pass_kernel<N1, N2, MODE, E, QC, PC, NTC, MINB, UG, AX, BASE>;
     // the dynamic shared-memory limit is a per-device function attribute: set it once per (kernel instance, device)
     static std::mutex mu;
     static bool configured[64] = {};
@@ -523,9 +525,12 @@ template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, in
 cudaError_t launch_one(const PassArgs& A, const LaunchPlan& L, cudaStream_t s) {
     constexpr bool kHasUG = MODE == rtepass::MODE_FIRST && QC != 0 && (QC / (PC ? PC : 1)) > 1;
     if constexpr (kHasUG)
-        if (A.g_uniform > 0.f) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, true, AX>(A, L, s);
+        if (A.g_uniform > 0.f && A.base == nullptr) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, true, AX>(A, L, s);
     PassArgs B = A;
     B.g_uniform = 0.f;                 // every other instance builds and reads the N+1-number table
+    // specialised FIRST kernels with a fused Runge-Kutta combination (PassArgs::base): a separate instance, N+1-number table
+    if constexpr (MODE == rtepass::MODE_FIRST && QC != 0)
+        if (A.base != nullptr) return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, false, AX, true>(B, L, s);
     return launch_one_impl<N1, N2, MODE, E, QC, PC, NTC, MINB, false, AX>(B, L, s);
 }
 
@@ -603,27 +608,52 @@ bool build_cpl_table(int dim, int N, int axis, int P, int n, double dx, double s
     return true;
 }
 
-// (re)build the alternative-step tables: Euler updates with time step dt_alt on the same context
+constexpr double kRkAlpha[2] = {0.25, 2.0 / 3.0};      // SSP-RK3: u2 = 3/4 u + 1/4 E(u1), u' = 1/3 u + 2/3 E(u2)
+
+int upload_cpl(rte_ctx* c, CplEntry** dst, int axis, double scale) {
+    AxisTables& T = c->ax[axis];
+    std::vector<CplEntry> flat;
+    if (!build_cpl_table(c->grid.dim, c->N, axis, c->P, T.n, c->dx, scale, flat, nullptr))
+        return fail(c, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
+    if (!*dst) CUDA_TRY(c, cudaMalloc((void**)dst, flat.size() * sizeof(CplEntry) + 16));
+    CUDA_TRY(c, cudaMemcpyAsync(*dst, flat.data(), flat.size() * sizeof(CplEntry), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));     // flat is about to go out of scope
+    return RTE_OK;
+}
+
+// (re)build the alternative-step tables: Euler updates with time step dt_alt on the same context (+ their RK-scaled copies)
 int set_alt_dt(rte_ctx* c, float dt_alt) {
     if (c->dt_alt == dt_alt) return RTE_OK;
     for (int a = 0; a < c->grid.dim; ++a) {
-        AxisTables& T = c->ax[a];
-        std::vector<CplEntry> flat;
-        if (!build_cpl_table(c->grid.dim, c->N, a, c->P, T.n, c->dx, -(double)c->c * (double)dt_alt, flat, nullptr))
-            return fail(c, RTE_EUNSUPPORTED, "coupling fan-in exceeds the kernel's table size");
-        if (!T.cpl_alt) CUDA_TRY(c, cudaMalloc((void**)&T.cpl_alt, flat.size() * sizeof(CplEntry) + 16));
-        CUDA_TRY(c, cudaMemcpyAsync(T.cpl_alt, flat.data(), flat.size() * sizeof(CplEntry), cudaMemcpyHostToDevice, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        int rc = upload_cpl(c, &c->ax[a].cpl_alt, a, -(double)c->c * (double)dt_alt);
+        for (int j = 0; j < 2 && rc == RTE_OK; ++j)
+            rc = upload_cpl(c, &c->ax[a].cpl_rk[1][j], a, -(double)c->c * (double)dt_alt * kRkAlpha[j]);
+        if (rc != RTE_OK) return rc;
     }
     c->dt_alt = dt_alt;
+    return RTE_OK;
+}
+
+// the RK-scaled copies of the main tables, built at the first SSP-RK3 step
+int ensure_rk_tables(rte_ctx* c) {
+    if (c->ax[0].cpl_rk[0][0]) return RTE_OK;
+    for (int a = 0; a < c->grid.dim; ++a)
+        for (int j = 1; j >= 0; --j) {                  // [0][0] last: it is the "built" marker
+            const int rc = upload_cpl(c, &c->ax[a].cpl_rk[0][j], a, -(double)c->c * (double)c->dt * kRkAlpha[j]);
+            if (rc != RTE_OK) return rc;
+        }
     return RTE_OK;
 }
 
 // One sweep of the per-axis pass kernels, out = F(in) with F chosen by `kind` (PassKind above): the forward-Euler update
 // of eq.(11) with the source at t_src, the steady-state operator, or the exponential Euler update.
 // amp_dev (optional): device location of c dt f(t) for this sweep (CUDA-graph replay), instead of the host value.
+// rk_stage (KIND_STEP / KIND_ALT only): 0 = plain; 1, 2 = the scaled update of an SSP-RK3 stage with the combination fused in,
+//   out = alpha E(in) + (1 - alpha) rk_base,  alpha = 1/4, 2/3 (tables scaled by alpha; the FIRST pass adds (1 - alpha) rk_base).
 int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKind kind = KIND_STEP,
-                 cudaEvent_t* ev = nullptr, const int* halt = nullptr, const float* amp_dev = nullptr) {
+                 cudaEvent_t* ev = nullptr, const int* halt = nullptr, const float* amp_dev = nullptr, int rk_stage = 0,
+                 const float2* rk_base = nullptr) {
+    const float alpha = rk_stage ? (float)kRkAlpha[rk_stage - 1] : 1.f;
     const int naxes = c->grid.dim;
     const int fa = c->first_axis;
     // the FIRST pass stores, the others add to what it stored: it goes first
@@ -632,10 +662,15 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
         PassArgs A{};
         A.psi = in; A.acc = out;
         A.cpl = kind == KIND_OPER ? c->ax[axis].cpl_op : (kind == KIND_ALT ? c->ax[axis].cpl_alt : c->ax[axis].cpl);
+        if (rk_stage) A.cpl = c->ax[axis].cpl_rk[kind == KIND_ALT ? 1 : 0][rk_stage - 1];
         A.tw = c->ax[axis].tw;
         A.sa = c->sa; A.ss = c->ss; A.gm = c->gm; A.deg = c->deg;
         A.cdt = kind == KIND_OPER ? -1.f : (kind == KIND_ALT ? c->c * c->dt_alt : (kind == KIND_STREAM ? 0.f : c->c * c->dt));
         A.ident = (kind == KIND_OPER || kind == KIND_STREAM) ? 0.f : 1.f;      // STREAM: s_l = 0 - 0 sigma_l = 0
+        if (rk_stage) {                 // the diagonal table is linear in (ident, cdt): alpha s_l = alpha - (alpha c dt) sigma_l
+            A.ident *= alpha; A.cdt *= alpha;
+            if (axis == fa) { A.base = rk_base; A.beta = 1.f - alpha; }
+        }
         A.expo = kind == KIND_EXP ? 1 : 0;
         A.first = axis == fa ? 1 : 0;
         A.first_axis = fa;
@@ -649,9 +684,9 @@ int euler_update(rte_ctx* c, const float2* in, float2* out, double t_src, PassKi
         if (nt_override > 0) L.nt = nt_override;
         const int n = c->ax[axis].n;
         if (A.first && c->src_kind != 0 && kind == KIND_ALT) {
-            A.src_amp = c->c * c->dt_alt * c->alt_src;
+            A.src_amp = c->c * c->dt_alt * c->alt_src * alpha;
         } else if (A.first && c->src_kind != 0 && kind != KIND_OPER && kind != KIND_STREAM) {
-            A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src));
+            A.src_amp = (float)((double)c->c * (double)c->dt * source_time_factor(c, t_src) * (double)alpha);
             A.src_amp_dev = amp_dev;
             if (amp_dev) A.src_amp = 1.f;      // non-zero: the kernel reads the device value
         }
@@ -824,43 +859,32 @@ float2* extra_field(const rte_ctx* c, int i) {
 }
 
 // One SSP-RK3 step on explicit buffers with the alternative time step and a constant source factor (KIND_ALT):
-// Y = RK3(X); X is only read, Z is scratch.
+// Y = RK3(X); X is only read, Z is scratch.  The stage combinations are fused into the passes (euler_update rk_stage).
 int rk3_alt(rte_ctx* c, const float2* X, float2* Y, float2* Z, const int* halt) {
-    const size_t n4 = (size_t)c->G * c->Cp / 4;
-    const int gb = grid_for((long long)n4, 256);
-    int rc = euler_update(c, X, Y, 0.0, KIND_ALT, nullptr, halt);
+    int rc = euler_update(c, X, Y, 0.0, KIND_ALT, nullptr, halt);                       // u1 = E(u)
     if (rc != RTE_OK) return rc;
-    rc = euler_update(c, Y, Z, 0.0, KIND_ALT, nullptr, halt);
+    rc = euler_update(c, Y, Z, 0.0, KIND_ALT, nullptr, halt, nullptr, 1, X);            // u2 = 3/4 u + 1/4 E(u1)
     if (rc != RTE_OK) return rc;
-    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Z, (const float4*)X, 0.75f, 0.25f, n4, halt);
-    rc = euler_update(c, Z, Y, 0.0, KIND_ALT, nullptr, halt);
-    if (rc != RTE_OK) return rc;
-    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Y, (const float4*)X, (float)(1.0 / 3.0), (float)(2.0 / 3.0), n4, halt);
-    c->launches += 2;
-    return RTE_OK;
+    return euler_update(c, Z, Y, 0.0, KIND_ALT, nullptr, halt, nullptr, 2, X);          // u' = 1/3 u + 2/3 E(u2)
 }
 
 // SSP-RK3 (Shu-Osher form, not the paper's integrator):
 //   u1 = E(u^n; t_n),  u2 = 3/4 u^n + 1/4 E(u1; t_n + dt),  u^{n+1} = 1/3 u^n + 2/3 E(u2; t_n + dt/2)
+// The convex combinations are fused into the passes: the tables of stages 2 and 3 carry the factor 1/4 (2/3), and their FIRST
+// pass adds 3/4 (1/3) u^n while it stores — no separate state-wide combination kernels.
 int one_step_ssprk3(rte_ctx* c) {
     float2* Z = extra_field(c, 0);
     if (!Z) return fail(c, RTE_EINVAL, "rte_step_ssprk3 needs one state-sized field of extra workspace (rte_set_extra_workspace)");
+    int rc = ensure_rk_tables(c);
+    if (rc != RTE_OK) return rc;
     float2 *X = c->psi, *Y = c->part;
     const double tn = (double)c->steps * (double)c->dt, dt = (double)c->dt;
-    const size_t n4 = (size_t)c->G * c->Cp / 4;            // Cp is even and records are 8-byte pairs: G*Cp*4 B, /16
-    const size_t rem = ((size_t)c->G * c->Cp) % 4;
-    if (rem != 0) return fail(c, RTE_EUNSUPPORTED, "state size not a multiple of 16 bytes");
-    const int gb = grid_for((long long)n4, 256);
-    int rc = euler_update(c, X, Y, tn);
+    rc = euler_update(c, X, Y, tn);
     if (rc != RTE_OK) return rc;
-    rc = euler_update(c, Y, Z, tn + dt);
+    rc = euler_update(c, Y, Z, tn + dt, KIND_STEP, nullptr, nullptr, nullptr, 1, X);
     if (rc != RTE_OK) return rc;
-    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Z, (const float4*)X, 0.75f, 0.25f, n4);
-    rc = euler_update(c, Z, Y, tn + 0.5 * dt);
+    rc = euler_update(c, Z, Y, tn + 0.5 * dt, KIND_STEP, nullptr, nullptr, nullptr, 2, X);
     if (rc != RTE_OK) return rc;
-    k_axpby<<<gb, 256, 0, c->stream>>>((float4*)Y, (const float4*)X, (float)(1.0 / 3.0), (float)(2.0 / 3.0), n4);
-    c->launches += 2;
-    if (cudaGetLastError() != cudaSuccess) return fail(c, RTE_ECUDA, "CUDA: %s", "axpby launch failed");
     c->psi = Y; c->part = X;                                // X (u^n) is free now; Z stays the spare buffer
     c->steps += 1;
     return RTE_OK;
@@ -909,6 +933,7 @@ void free_ctx(rte_ctx* c) {
     if (!c) return;
     for (int a = 0; a < 3; ++a) {
         cudaFree(c->ax[a].cpl); cudaFree(c->ax[a].cpl_op); cudaFree(c->ax[a].cpl_alt); cudaFree(c->ax[a].tw);
+        for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) cudaFree(c->ax[a].cpl_rk[i][j]);
     }
     if (c->graph) cudaGraphExecDestroy(c->graph);
     cudaFree(c->graph_amp);

@@ -62,6 +62,8 @@ struct PassArgs {
                             // multiplies psi AND the streaming term, the source carries phi_1 (rte_step_exp)
     int first;              // MODE_RT kernels: 1 = FIRST, 0 = ACC
     int first_axis;         // axis of the FIRST pass (0 = x, 2 = z): how the source box maps onto its pencils
+    const float2* base;     // optional (FIRST pass): the store becomes  new = (scaled Euler update) + beta * base  — a Runge-Kutta
+    float beta;             // stage combination fused into the pass (the scaling itself is in the tables: rte_lib.cu euler_update)
     const int* halt;        // optional device flag: non-zero => the launch does nothing (Krylov solver, converged early)
     const float2* tw;       // generic kernels: forward twiddles exp(-2 pi i j / n) of this axis, n entries (global)
     int nsig;               // N + 1 degrees
@@ -141,6 +143,11 @@ __device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
                  "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+
+// L2 prefetch of a contiguous global range (no destination in shared memory, nothing to wait for)
+__device__ __forceinline__ void tma_prefetch_l2(const void* gmem_src, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
 }
 
 // ---- tile geometry ------------------------------------------------------------------------------------------------------
@@ -462,12 +469,12 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, long lo
 // ---- tail, specialised kernels: inverse first factor in registers, then one store / vector reduction per element ---------
 // (the coupling was applied in phase 1; every thread owns its column, so there is no barrier and no neighbour data)
 // FIRST: r holds the column's own psi (loaded by tail_load, the first task's before the phase-2 barrier).
-template <int N1, int N2, int QC, int PC, int AX>
-__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]);
+template <int N1, int N2, int QC, int PC, int AX, bool BASE = false>
+__device__ __forceinline__ void tail_load(const PassArgs& A, const float* sig, long long base, int task, float2 (&r)[N1]);
 
 // LATE (FIRST instances whose register budget cannot hold the psi column next to the transform's): the re-read is issued
 // after the inverse DFT instead of before it; the higher occupancy of those instances hides its latency.
-template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG, int AX, bool LATE = false>
+template <int N1, int N2, int MODE, int QC, int PC, bool STACKED, bool UG, int AX, bool LATE = false, bool BASE = false>
 __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile, const float* sig, long long base, int task,
                                           long long pencil0, float2 (&r)[N1]) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
@@ -482,7 +489,7 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
     if (MODE == MODE_FIRST) rtefft::dft_inv_swap<N1>(v);      // register pressure: see rte_fft.cuh
     else rtefft::dft_inv<N1>(v);
-    if (MODE == MODE_FIRST && LATE) tail_load<N1, N2, QC, PC, AX>(A, base, task, r);
+    if (MODE == MODE_FIRST && LATE) tail_load<N1, N2, QC, PC, AX, BASE>(A, sig, base, task, r);
     // x pass (AX == 0): the pencil is contiguous (cell stride 1, pencil stride n), so every address of the column is the
     // base plus a compile-time offset and folds into the instruction's immediate field
     float2* sp = AX == 0 ? A.acc + (base + (long long)t * n + b) * P + p
@@ -496,7 +503,14 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
         const int i0 = __ldg(A.deg + 2 * p) * pl + t * pt + b, i1 = __ldg(A.deg + 2 * p + 1) * pl + t * pt + b;
         const SourceRow src(A, AX, pencil0 + t, p);
         // (the source test is hoisted out of the element loops: almost every pencil lies outside the source box)
-        if (UG) {
+        if (BASE) {                 // r already holds s_l psi + beta base (tail_load)
+#pragma unroll
+            for (int a = 0; a < N1; ++a) {
+                float2 e = rtefft::cadd(r[a], v[a]);
+                src.add(a * N2 + b, e);
+                store(a, e);
+            }
+        } else if (UG) {
             const float2* ab = reinterpret_cast<const float2*>(sig) + t * n + b;
             float g0 = 1.f, g1 = 1.f;
             for (int l = __ldg(A.deg + 2 * p); l > 0; --l) g0 *= A.g_uniform;          // g^l by repeated multiplication (R16)
@@ -539,15 +553,31 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
 }
 
 // the psi re-read of one FIRST tail task, issued as early as possible
-template <int N1, int N2, int QC, int PC, int AX>
-__device__ __forceinline__ void tail_load(const PassArgs& A, long long base, int task, float2 (&r)[N1]) {
+// BASE (x pass with a fused Runge-Kutta combination): the base field is loaded here too and folded in at once,
+//   r = s_l psi + beta base   (s_l from the diagonal table, complete since the barrier after phase 1),
+// so that both streams are in flight before the phase-2 barrier and the tail only adds the streaming term.
+template <int N1, int N2, int QC, int PC, int AX, bool BASE>
+__device__ __forceinline__ void tail_load(const PassArgs& A, const float* sig, long long base, int task, float2 (&r)[N1]) {
     constexpr int P = PC, Q = QC;
     const int b = task / Q, q = task - b * Q;
     const int t = q / P, p = q - t * P;
     if (AX == 0) {          // x pass: compile-time offsets (see tail_spec)
-        const float2* lp = A.psi + (base + (long long)t * (N1 * N2) + b) * P + p;
+        const long long off = (base + (long long)t * (N1 * N2) + b) * P + p;
+        const float2* lp = A.psi + off;
 #pragma unroll
         for (int a = 0; a < N1; ++a) r[a] = lp[a * (N2 * P)];
+        if (BASE) {
+            constexpr int n = N1 * N2;
+            constexpr int pl = sig_pitch_l(n, QC / PC), pt = sig_pitch_t(n);
+            const int i0 = __ldg(A.deg + 2 * p) * pl + t * pt + b, i1 = __ldg(A.deg + 2 * p + 1) * pl + t * pt + b;
+            const float2* xp = A.base + off;
+            float2 x[N1];
+#pragma unroll
+            for (int a = 0; a < N1; ++a) x[a] = xp[a * (N2 * P)];
+#pragma unroll
+            for (int a = 0; a < N1; ++a)
+                r[a] = make_float2(fmaf(sig[i0 + a * N2], r[a].x, A.beta * x[a].x), fmaf(sig[i1 + a * N2], r[a].y, A.beta * x[a].y));
+        }
     } else {
         const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
         const float2* lp = A.psi + (base + (long long)t * A.stride_t + (long long)b * A.stride_i) * P + p;
@@ -625,6 +655,14 @@ __device__ __forceinline__ void tail_generic(const PassArgs& A, const float2* ti
         }
     }
     if (first) {
+        if (A.base != nullptr) {          // Runge-Kutta stage combination fused into the store
+            const float2* bp = A.base + gi;
+#pragma unroll
+            for (int a = 0; a < N1; ++a) {
+                const float2 x = ldg64(bp, stepB * a);
+                r[a].x = fmaf(A.beta, x.x, r[a].x); r[a].y = fmaf(A.beta, x.y, r[a].y);
+            }
+        }
 #pragma unroll
         for (int a = 0; a < N1; ++a) stg64(sp, stepB * a, r[a]);
     } else {
@@ -645,7 +683,7 @@ constexpr int generic_max_threads(int N1, int N2) {
 // UG (specialised FIRST kernels only): uniform g, the 2-number diagonal table (build_sig); the host picks the instance.
 // AX (specialised kernels): the axis of the pass — x tiles of several pencils use the stacked layout, x / y have pure
 // coupling slots, the FIRST pass maps the source box onto its pencils by AX.
-template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0>
+template <int N1, int N2, int MODE, int E, int QC, int PC, int NTC, int MINB, bool UG = false, int AX = 0, bool BASE = false>
 __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB) pass_kernel(const __grid_constant__ PassArgs A) {
     extern __shared__ __align__(128) float2 smem[];
     constexpr int n = N1 * N2;
@@ -690,6 +728,14 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
         }
         __syncthreads();
         tile_tma_load<N1, N2, QC, PC, STACKED>(A, tile, base, bar, tid, nt);
+        if constexpr (BASE && AX == 0) {
+            // the Runge-Kutta base field of this (contiguous) x tile is read in the tail: bring it into L2 now, so that those
+            // loads cost an L2 hit like the psi re-read instead of a DRAM round trip each
+            constexpr unsigned tile_bytes = (unsigned)n * QC * 8u;
+            constexpr unsigned piece = tile_bytes % 16384u == 0 ? 16384u : (tile_bytes % 4096u == 0 ? 4096u : tile_bytes);
+            for (unsigned j = tid; j < tile_bytes / piece; j += nt)
+                tma_prefetch_l2(reinterpret_cast<const char*>(A.base + base * PC) + (size_t)j * piece, piece);
+        }
         if (MODE == MODE_FIRST) build_sig<N1, N2, MAXC>(A, sig, cells, tid, nt);                 // read in the tail, two barriers later
     } else {
         if (first || A.expo) build_sig<N1, N2>(A, sig, base, valid, tid, nt);
@@ -702,14 +748,14 @@ __global__ void __launch_bounds__(NTC ? NTC : generic_max_threads(N1, N2), MINB)
         // FIRST: the first tail task's psi re-read is issued BEFORE the barrier and flies while the slower warps finish
         // phase 2 (the loads depend on nothing in shared memory)
         constexpr bool LATE = MODE == MODE_FIRST && 65536 / ((NTC ? NTC : 1) * MINB) < 80;
-        if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX>(A, base, tid, r);
+        if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX, BASE>(A, sig, base, tid, r);
         __syncthreads();
-        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE>(A, tile, sig, base, tid, pencil0, r);
+        tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE, BASE>(A, tile, sig, base, tid, pencil0, r);
 #pragma unroll 1
         for (int task = tid + nt; task < Q * N2; task += nt) {
             float2 r2[N1];
-            if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX>(A, base, task, r2);
-            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE>(A, tile, sig, base, task, pencil0, r2);
+            if (MODE == MODE_FIRST && !LATE) tail_load<N1, N2, QC, PC, AX, BASE>(A, sig, base, task, r2);
+            tail_spec<N1, N2, MODE, QC, PC, STACKED, UG, AX, LATE, BASE>(A, tile, sig, base, task, pencil0, r2);
         }
     } else {
         __syncthreads();
