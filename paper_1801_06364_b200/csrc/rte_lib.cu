@@ -1735,18 +1735,23 @@ int rte_media_lognormal(const rte_grid* grid, float dx, uint64_t seed, float mea
     const float s_cells = corr_len / 1.41421356237f / dx;
     const int R = (int)std::ceil(4.0f * s_cells);
     const float inv2s2 = 1.0f / (2.0f * s_cells * s_cells);
+    cudaError_t e = cudaSuccess;
+    auto check = [&]() { const cudaError_t l = cudaGetLastError(); if (e == cudaSuccess) e = l; };      // every launch, first error kept
     k_white_noise<<<gb, 256, 0, s>>>(out_dev, G, (unsigned long long)seed);
+    check();
     float* a = out_dev;
     float* b = scratch_dev;
     for (int axis = 0; axis < grid->dim; ++axis) {
         k_blur_axis<<<gb, 256, 0, s>>>(b, a, grid->nx, grid->ny, grid->nz, axis, R, inv2s2);
+        check();
         float* t = a; a = b; b = t;
     }
     if (a != out_dev) cudaMemcpyAsync(out_dev, a, (size_t)G * sizeof(float), cudaMemcpyDeviceToDevice, s);
     k_moments<<<gb, 256, 0, s>>>(out_dev, G, red);
+    check();
     k_lognormal_finish<<<gb, 256, 0, s>>>(out_dev, G, red, mean, sigma_log);
-    cudaError_t e = cudaGetLastError();
-    cudaStreamSynchronize(s);
+    check();
+    { const cudaError_t l = cudaStreamSynchronize(s); if (e == cudaSuccess) e = l; }
     cudaFree(red);
     return e == cudaSuccess ? RTE_OK : RTE_ECUDA;
 }
