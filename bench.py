@@ -352,7 +352,9 @@ def roofline_of(cfg, res, peak, peak_kind):
             "bytes_per_coefficient_cell_step": per_step / (cfg.C * cfg.G),
             "whole_step": {"algorithmic_bytes": per_step, "achieved_gbs": step_gbs, "frac": step_gbs / peak,
                            "frac_of_nominal_8000": step_gbs / 8000.0},
-            "kernels": kernels}
+            "kernels": kernels,
+            "note": "fractions are of the HBM roofline; the FIRST (x) pass is limited by the SM load/store data path (ncu: 65-70 % "
+                    "busy at 16 warps per SM, profiles/), the accumulating passes by HBM"}
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
