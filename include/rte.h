@@ -149,7 +149,8 @@ int rte_set_source_host(rte_ctx* ctx, const float* w_host, const float* S_host, 
  * (eq.(9),(12)) and stores psi(1 - c dt sigma_l) + c dt q - c dt T_x into the second state buffer, the other axes add
  * their -c dt T_a to it; the buffers then trade places.  Results are bit-reproducible from run to run.
  * Grids whose state is at most 24 MB (L2-resident, launch-bound) replay the same launches from a CUDA graph, 32 steps
- * per replay; the results are identical to the eager path.  Grids without specialised kernels (anything but the BASELINE
+ * per replay (captured on a private stream by the first call that asks for >= 4 steps; the caller's stream must not be
+ * capturing then); the results are identical to the eager path.  Grids without specialised kernels (anything but the BASELINE
  * shapes) time a few block sizes per axis at the context's first sweep and keep the fastest: that first call synchronises
  * the stream once; results do not depend on the choice. */
 int rte_step(rte_ctx* ctx, int nsteps);
