@@ -494,6 +494,7 @@ LaunchPlan plan_pass(const rte_ctx* c, int axis, PassArgs& A, PassKind kind) {
     L.blocks = groups * A.tiles_per_group;
     L.smem = pass_smem(n, L.TP * P, L.TP, c->N + 1, diag);
     if (L.spec >= 0 && axis == 0 && L.TP > 1) L.smem += (size_t)L.TP * (P % 16) * sizeof(float2);   // stacked-layout padding
+    if (L.spec >= 0 && axis == 0 && L.TP == 1 && P % 16 != 0) L.smem += 32 * 2 * sizeof(float2);   // block gaps (Geo::PADB), N1 <= 32
     return L;
 }
 

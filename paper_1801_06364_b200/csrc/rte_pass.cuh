@@ -159,7 +159,15 @@ struct Geo {
     static constexpr int TPC = QC / (PC ? PC : 1);
     static constexpr int pad = (STACKED && TPC > 1) ? (PC % 16) : 0;
     static constexpr int SI = STACKED ? PC : QC;             // 0 when run-time
-    static constexpr int ST = STACKED ? n * PC + pad : PC;
+    // One-pencil stacked tiles whose rows are not a multiple of 16 elements (P_5: 18 pairs): the phase-2 tasks of a half-warp
+    // straddle two k1 blocks, N2 rows = N2*P elements apart — a multiple of 16 banks, i.e. a 2-way conflict.  A gap of PADB
+    // elements after every block of N2 rows shifts consecutive blocks by 2 banks (ncu, cfg3 x pass: 20 % of the shared
+    // wavefronts were conflicts).  SA = element stride between the rows i and i + N2.
+    // (the interleaved y / z tiles of such records, rows of Q = 36 elements, have the same conflicts; padding them was measured
+    // and changes nothing: those passes are HBM-bound)
+    static constexpr int PADB = (STACKED && TPC == 1 && PC % 16 != 0 && (N2 * PC) % 16 == 0) ? 2 : 0;
+    static constexpr int SA = N2 * SI + PADB;                // 0 when run-time (SI = 0, PADB = 0)
+    static constexpr int ST = STACKED ? n * PC + pad + N1 * PADB : PC;
     static constexpr int tile_elems = STACKED ? TPC * ST : n * QC;
 };
 
@@ -168,7 +176,12 @@ template <int N1, int N2, int QC, int PC, bool STACKED>
 __device__ __forceinline__ void tile_tma_load(const PassArgs& A, float2* tile, long long base, unsigned long long* bar, int tid,
                                               int nt) {
     using G = Geo<N1, N2, QC, PC, STACKED>;
-    if (STACKED) {
+    if (STACKED && G::PADB != 0) {
+        // one pencil, one copy per block of N2 rows (N2*P*8 contiguous bytes) into its padded place
+        constexpr unsigned blk_bytes = (unsigned)N2 * PC * 8u;
+        for (int a = tid; a < N1; a += nt)
+            tma_load_1d(tile + a * G::SA, reinterpret_cast<const char*>(A.psi + base * PC) + (size_t)a * blk_bytes, blk_bytes, bar);
+    } else if (STACKED) {
         // TP whole pencils of n*P*8 contiguous bytes each, issued as 16 KB pieces by different threads
         constexpr unsigned pen_bytes = (unsigned)G::n * PC * 8u;
         constexpr unsigned piece = pen_bytes % 16384u == 0 ? 16384u : (pen_bytes % 4096u == 0 ? 4096u : pen_bytes);
@@ -248,6 +261,7 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
     const int Q = QC ? QC : A.TP * P;
     const int SI = G::SI ? G::SI : Q;
     const int ST = G::ST ? G::ST : P;
+    const int SA = G::SA ? G::SA : N2 * SI;                  // stride between the rows i and i + N2
     const unsigned long long stepB = (unsigned long long)N2 * (unsigned)A.stride_i * (unsigned)P * 8u;
 #pragma unroll 1
     for (int task = tid; task < Q * N2; task += nt) {
@@ -276,7 +290,7 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
                 float2 u = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
-                    const float2 d = srow[e][(a * N2) * SI];
+                    const float2 d = srow[e][a * SA];
                     // slots [0, NPURE) hold purely diagonal (x pass) / purely off-diagonal (y pass) blocks: one packed FMA
                     if (e >= NPURE || PURE_DIAG) u = rtefft::cfma_diag(wd[e].x, wd[e].y, d, u);
                     if (e >= NPURE || !PURE_DIAG) u = rtefft::cfma_swap(ws[e].x, ws[e].y, d, u);
@@ -297,7 +311,7 @@ __device__ __forceinline__ void phase_fwd1(const PassArgs& A, float2* tile, cons
         }
         rtefft::dft_fwd<N1>(v);
 #pragma unroll
-        for (int k1 = 0; k1 < N1; ++k1) col[k1 * N2 * SI] = v[k1];
+        for (int k1 = 0; k1 < N1; ++k1) col[k1 * SA] = v[k1];
     }
 }
 
@@ -316,7 +330,7 @@ __device__ __forceinline__ void phase_mid(const PassArgs& A, float2* tile, int t
 #pragma unroll 1
     for (int task = tid; task < Q * N1; task += nt) {
         const int k1 = task / Q, q = task - k1 * Q;
-        float2* row = tile + (k1 * N2) * SI + col_offset<G, STACKED>(q, P);
+        float2* row = tile + k1 * (G::SA ? G::SA : N2 * SI) + col_offset<G, STACKED>(q, P);
         float2 v[N2], w[N2];
 #pragma unroll
         for (int b = 0; b < N2; ++b) v[b] = row[b * SI];
@@ -486,7 +500,7 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
     const float2* col = tile + b * SI + t * ST + p;
     float2 v[N1];
 #pragma unroll
-    for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[(k1 * N2) * SI];
+    for (int k1 = 0; k1 < N1; ++k1) v[k1] = col[k1 * G::SA];
     if (MODE == MODE_FIRST) rtefft::dft_inv_swap<N1>(v);      // register pressure: see rte_fft.cuh
     else rtefft::dft_inv<N1>(v);
     if (MODE == MODE_FIRST && LATE) tail_load<N1, N2, QC, PC, AX, BASE>(A, sig, base, task, r);
