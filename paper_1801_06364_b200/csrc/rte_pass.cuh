@@ -446,7 +446,9 @@ __device__ __forceinline__ void build_sig(const PassArgs& A, float* sig, const S
         const int t = j / n, i = j - t * n;
         const float sa = c.sa[k], ss = c.ss[k], g = c.g[k];
         if (ug) {
-            ab[j] = make_float2(A.ident - A.cdt * (sa + ss), A.cdt * ss);
+            // pitch n + 1 per pencil: the lanes of a warp read the entries of TP pencils at the same position, and n is a
+            // multiple of the 16 eight-byte banks (ncu, cfg2 x pass: a 4-way conflict on every table read)
+            ab[t * (n + 1) + i] = make_float2(A.ident - A.cdt * (sa + ss), A.cdt * ss);
             continue;
         }
         float pw = 1.f;
@@ -525,7 +527,7 @@ __device__ __forceinline__ void tail_spec(const PassArgs& A, const float2* tile,
                 store(a, e);
             }
         } else if (UG) {
-            const float2* ab = reinterpret_cast<const float2*>(sig) + t * n + b;
+            const float2* ab = reinterpret_cast<const float2*>(sig) + t * (n + 1) + b;
             float g0 = 1.f, g1 = 1.f;
             for (int l = __ldg(A.deg + 2 * p); l > 0; --l) g0 *= A.g_uniform;          // g^l by repeated multiplication (R16)
             for (int l = __ldg(A.deg + 2 * p + 1); l > 0; --l) g1 *= A.g_uniform;
