@@ -359,9 +359,9 @@ def roofline_of(cfg, res, peak, peak_kind):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each axis kernel, from the committed ncu --set full
 # captures under profiles/ (filled in from the capture named there; None until one exists for that workload)
-TRAFFIC_NCU = {"cfg4": {0: 29829106000, 1: 43428733000, 2: 43431895999},       # profiles/r2q_summary.md §3 (ncu --set full,
-               "cfg3": {0: 5007254000, 1: 7194439000, 2: 7201378000},          # one launch per axis kernel)
-               "cfg2": {0: 246207232, 1: 344941056, 2: 346196479}}
+TRAFFIC_NCU = {"cfg4": {0: 29826771000, 1: 43432582000, 2: 43432402000},       # profiles/r2r_summary.md §3 (ncu --set full,
+               "cfg3": {0: 5007557999, 1: 7193890000, 2: 7201423999},          # one launch per axis kernel)
+               "cfg2": {0: 246775552, 1: 345737728, 2: 346095360}}
 
 
 def max_over_ranks(ms, dist, device):
